@@ -1,0 +1,422 @@
+"""Oracle: plain, slow fp64 CPU restatement of one nsCouette predictor-corrector step.
+
+TEST INFRASTRUCTURE ONLY.  Nothing in the product path (the package
+``paper_1908_00587_b200``) may import this module; only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference``
+legs do.  It shares no code, table or constant with the CUDA path.
+
+What it restates (citations are PAPER.md:<line>, or
+DESIGN.md reading R#):
+
+* PAPER.md:36      cylindrical coordinates, primitive variables (u_r, u_theta, u_z, p, T)
+* PAPER.md:42      Fourier-Galerkin in theta and z; 9-point finite differences in r on a
+                   radial grid selected at run time
+* PAPER.md:44      axial periodicity
+* PAPER.md:46      predictor-corrector time integration, implicit linear terms
+* PAPER.md:48-50   Boussinesq heat transfer, negative radial temperature gradient, gravity || z
+* PAPER.md:64      linear terms solved independently per Fourier mode; nonlinear terms need
+                   all modes of a radial node
+* PAPER.md:100     the basic state depends on r only (circular Couette flow, conductive T)
+* PAPER.md:108     time unit d^2/nu
+
+The paper prints no equations; every numerical choice is a DESIGN.md reading (R1..R15,
+taken from SURVEY.md 8(c) S1..S15).  Layout of every spectral field: complex128 array
+``[N_r, M+1, 2K+1]``, ``m = 0..M``, ``k index = k + K``, ``j = 0`` at the inner wall.
+
+Transforms are naive O(N^2) sums written as matrix products with explicit root-of-unity
+tables (``dft="naive"``).  ``dft="fft"`` swaps those sums for numpy's FFT routines (a
+library primitive standing for the same sums; pinned to the naive sums in
+tests/test_oracle_transforms.py) so that the large configurations finish.
+
+Linear solves are dense Gaussian elimination with partial pivoting after row
+equilibration (LAPACK ``gesv`` through ``numpy.linalg.solve`` on row-scaled matrices).
+
+Parity unpinned (defined by the algorithm only): the pressure field,
+the O(dt^2) tangential wall slip, and the aliased extreme modes |k| = K, m = M.
+"""
+from __future__ import annotations
+
+import dataclasses
+import numpy as np
+
+LD = np.longdouble
+
+
+# --------------------------------------------------------------------------------------
+# parameters
+# --------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class Params:
+    """Arguments of ``nsc_create`` (BASELINE.json north_star; "number of
+    points, modes ... rotation rates")."""
+    N_r: int
+    M: int                 # azimuthal modes m = 0..M
+    K: int                 # axial modes k = -K..K
+    eta: float             # radius ratio r_i / r_o
+    alpha: float           # axial base wavenumber, kappa = k * alpha
+    k_theta0: int          # azimuthal base wavenumber, n = m * k_theta0
+    Re_i: float
+    Re_o: float
+    Ra: float = 0.0
+    Pr: float = 1.0
+    grid: int = 1          # 0 uniform, 1 Chebyshev-Gauss-Lobatto (R2)
+    n_theta: int = 0       # physical grid; 0 => 3M (R4)
+    n_z: int = 0           # physical grid; 0 => 3K (R4)
+    c: float = 0.5         # implicitness (R10)
+
+    def __post_init__(self):
+        if self.n_theta == 0:
+            self.n_theta = 3 * self.M
+        if self.n_z == 0:
+            self.n_z = 3 * self.K
+
+    @property
+    def heated(self) -> bool:      # R13: temperature on iff Ra != 0
+        return self.Ra != 0.0
+
+
+# --------------------------------------------------------------------------------------
+# O1 radial grid, O2 finite-difference tables
+# --------------------------------------------------------------------------------------
+def radial_grid(N_r: int, eta: float, kind: int, dtype=np.float64):
+    """O1.  Gap d = r_o - r_i = 1, r_i = eta/(1-eta) (R1; PAPER.md:108 fixes d as length
+    unit).  kind 0: uniform; kind 1: Chebyshev-Gauss-Lobatto clustering (R2)."""
+    eta = LD(eta)
+    r_i = eta / (1 - eta)
+    j = np.arange(N_r, dtype=LD)
+    if kind == 0:
+        r = r_i + j / (N_r - 1)
+    elif kind == 1:
+        r = r_i + (1 - np.cos(_pi_ld() * j / (N_r - 1))) / 2
+    else:
+        raise ValueError("radial grid kind must be 0 or 1")
+    return r.astype(dtype)
+
+
+def _pi_ld():
+    return LD(4) * np.arctan(LD(1))
+
+
+def stencil_start(j: int, N_r: int, npt: int = 9) -> int:
+    """R3: 9-node window centred inside, shifted (one-sided) at the walls."""
+    return min(max(j - npt // 2, 0), N_r - npt)
+
+
+def fd_tables(r_ld, npt: int = 9):
+    """O2.  Dense D1, D2 [N_r, N_r] in long double: derivatives at r_j of the degree-8
+    Lagrange basis on the stencil S(j) ("stencil-length ... nine points").
+
+    l != j:  l_l'(x_j)  = prod_{q != l,j}(x_j-x_q) / prod_{q != l}(x_l-x_q)
+             l_l''(x_j) = 2 l_l'(x_j) * sum_{q != l,j} 1/(x_j-x_q)
+    l == j:  l_j'(x_j)  = s1 = sum_{q != j} 1/(x_j-x_q)
+             l_j''(x_j) = s1^2 - sum_{q != j} 1/(x_j-x_q)^2
+    """
+    r_ld = np.asarray(r_ld, dtype=LD)
+    N = len(r_ld)
+    D1 = np.zeros((N, N), LD)
+    D2 = np.zeros((N, N), LD)
+    for j in range(N):
+        s = stencil_start(j, N, npt)
+        x = r_ld[s:s + npt]
+        jl = j - s
+        xj = x[jl]
+        for a in range(npt):
+            l = s + a
+            if a == jl:
+                inv = [1 / (xj - x[q]) for q in range(npt) if q != jl]
+                s1 = sum(inv, LD(0))
+                D1[j, l] = s1
+                D2[j, l] = s1 * s1 - sum((v * v for v in inv), LD(0))
+            else:
+                num = LD(1)
+                den = LD(1)
+                for q in range(npt):
+                    if q != a and q != jl:
+                        num *= xj - x[q]
+                    if q != a:
+                        den *= x[a] - x[q]
+                w1 = num / den
+                D1[j, l] = w1
+                D2[j, l] = 2 * w1 * sum((1 / (xj - x[q]) for q in range(npt)
+                                         if q != a and q != jl), LD(0))
+    return D1, D2
+
+
+def roots_of_unity(N: int):
+    """exp(2 pi i t / N), t = 0..N-1, evaluated in long double, rounded once (O3)."""
+    t = np.arange(N, dtype=LD)
+    ang = 2 * _pi_ld() * t / N
+    return np.cos(ang).astype(np.float64) + 1j * np.sin(ang).astype(np.float64)
+
+
+# --------------------------------------------------------------------------------------
+# the oracle
+# --------------------------------------------------------------------------------------
+class Oracle:
+    """One Taylor-Couette configuration; methods follow O3..O8 in SURVEY.md 8(c)."""
+
+    def __init__(self, p: Params, dft: str = "naive"):
+        self.p = p
+        self.dft = dft
+        N_r = p.N_r
+        r_ld = radial_grid(N_r, p.eta, p.grid, dtype=LD)
+        D1, D2 = fd_tables(r_ld)
+        inv_r = 1 / r_ld
+        L0 = D2 + inv_r[:, None] * D1                        # d2/dr2 + (1/r) d/dr
+        Gt = D1.copy()                                       # G~: D1 with wall rows zeroed
+        Gt[0, :] = 0
+        Gt[-1, :] = 0
+        Q = (D1 + np.diag(inv_r)) @ Gt                       # (D1 + 1/r) G~, product in LD
+        f64 = np.float64
+        self.r = r_ld.astype(f64)
+        self.D1, self.D2 = D1.astype(f64), D2.astype(f64)
+        self.L0, self.Gt, self.Q = L0.astype(f64), Gt.astype(f64), Q.astype(f64)
+        # wavenumbers (BASELINE.json (a): i*m*k_theta0 and i*k*alpha)
+        self.n = (np.arange(p.M + 1) * p.k_theta0).astype(f64)          # [M+1]
+        self.kappa = (np.arange(-p.K, p.K + 1) * p.alpha).astype(f64)   # [2K+1]
+        # O3 root tables, indexed by (m*a mod N_theta), (k*b mod N_z)
+        wt = roots_of_unity(p.n_theta)
+        wz = roots_of_unity(p.n_z)
+        m = np.arange(p.M + 1)[:, None]
+        a = np.arange(p.n_theta)[None, :]
+        k = np.arange(-p.K, p.K + 1)[:, None]
+        b = np.arange(p.n_z)[None, :]
+        self.Et = wt[(m * a) % p.n_theta]                    # [M+1, N_theta]
+        self.Ez = wz[(k * b) % p.n_z]                        # [2K+1, N_z]
+        self.cm = np.where(np.arange(p.M + 1) == 0, 1.0, 2.0)
+
+    # ---------------------------------------------------------------- O3 transforms
+    def to_physical(self, fh):
+        """u(theta_a, z_b) = Re[sum_k u^(0,k) e^{2 pi i k b/N_z}]
+                             + 2 Re[sum_{m>=1} sum_k u^(m,k) e^{2 pi i (m a/N_theta + k b/N_z)}].
+        fh: [..., M+1, 2K+1] -> real [..., N_theta, N_z]."""
+        p = self.p
+        if self.dft == "fft":
+            pad = np.zeros(fh.shape[:-2] + (p.n_theta // 2 + 1, p.n_z), complex)
+            kk = np.arange(-p.K, p.K + 1) % p.n_z
+            pad[..., :p.M + 1, kk] = fh
+            half = np.fft.ifft(pad, axis=-1) * p.n_z
+            return np.fft.irfft(half, n=p.n_theta, axis=-2) * p.n_theta
+        half = fh @ self.Ez                                   # sum over k -> [..., M+1, N_z]
+        half = half * self.cm[:, None]
+        return np.real(np.swapaxes(np.swapaxes(half, -1, -2) @ self.Et, -1, -2))
+
+    def from_physical(self, u):
+        """u^(m,k) = 1/(N_theta N_z) sum_{a,b} u(theta_a,z_b) e^{-2 pi i (m a/N_theta + k b/N_z)}
+        for 0 <= m <= M, |k| <= K; everything else discarded (truncation).
+        u: real [..., N_theta, N_z] -> [..., M+1, 2K+1]."""
+        p = self.p
+        if self.dft == "fft":
+            h = np.fft.fft(np.fft.rfft(u, axis=-2), axis=-1) / (p.n_theta * p.n_z)
+            kk = np.arange(-p.K, p.K + 1) % p.n_z
+            return h[..., :p.M + 1, :][..., kk]
+        t = np.conj(self.Et) @ u                              # sum over a -> [..., M+1, N_z]
+        return (t @ np.conj(self.Ez).T) / (p.n_theta * p.n_z)
+
+    # ---------------------------------------------------------------- O5 operators
+    def d_r(self, f):
+        """Radial derivative: sum_{l in S(j)} D1[j,l] f_l (N1)."""
+        return np.einsum("jl,lmk->jmk", self.D1, f)
+
+    def lap(self, f, shift: int):
+        """(L0 - diag((n+shift)^2/r^2 + kappa^2)) f.  shift = 0: scalar Laplacian L_s;
+        shift = +-1: L_+- acting on u_+- = u_r +- i u_theta (O5)."""
+        q = ((self.n[None, :, None] + shift) ** 2 / self.r[:, None, None] ** 2
+             + self.kappa[None, None, :] ** 2)
+        return np.einsum("jl,lmk->jmk", self.L0, f) - q * f
+
+    def divergence(self, ur, ut, uz):
+        """D1 u_r + u_r/r + (i n/r) u_theta + i kappa u_z (O5)."""
+        r = self.r[:, None, None]
+        return (self.d_r(ur) + ur / r + 1j * self.n[None, :, None] / r * ut
+                + 1j * self.kappa[None, None, :] * uz)
+
+    # ---------------------------------------------------------------- O4 nonlinear term
+    def nonlinear(self, ur, ut, uz, T=None, nodes=None):
+        """N = -(u.grad)u with the cylindrical curvature terms, + (Ra/Pr) T^ e_z, and
+        N_T = -(u.grad)T (N1..N6; convective form, R7).  Evaluated at every radial node
+        (walls included) or at the listed ``nodes`` only (same values; used for sampled
+        parity at the large configurations).  Returns [N_r, N_theta, N_z, (N_T)] spectral."""
+        p = self.p
+        fields = [ur, ut, uz] + ([T] if p.heated else [])
+        js = np.arange(p.N_r) if nodes is None else np.asarray(nodes)
+        i_n = 1j * self.n[None, :, None]
+        i_k = 1j * self.kappa[None, None, :]
+        rj = self.r[js][:, None, None]
+        ph, d_r, d_t, d_z = [], [], [], []
+        for f in fields:
+            fj = f[js]
+            ph.append(self.to_physical(fj))
+            d_r.append(self.to_physical(np.einsum("jl,lmk->jmk", self.D1[js], f)))
+            d_t.append(self.to_physical(i_n * fj))
+            d_z.append(self.to_physical(i_k * fj))
+        Ur, Ut, Uz = ph[0], ph[1], ph[2]
+
+        def adv(i):
+            return Ur * d_r[i] + (Ut / rj) * d_t[i] + Uz * d_z[i]
+
+        Nr = -(adv(0) - Ut * Ut / rj)
+        Nt = -(adv(1) + Ur * Ut / rj)
+        Nz = -adv(2)
+        out = [self.from_physical(Nr), self.from_physical(Nt), self.from_physical(Nz)]
+        if p.heated:
+            out[2] = out[2] + (p.Ra / p.Pr) * T[js]           # Boussinesq buoyancy (R8)
+            out.append(self.from_physical(-adv(3)))
+        return out
+
+    # ---------------------------------------------------------------- O6 sub-step
+    def _solve_rows(self, A, b):
+        """Dense LU with partial pivoting after row equilibration.  A [B,N,N] real,
+        b [B,N] complex."""
+        s = 1.0 / np.abs(A).max(axis=2)
+        return np.linalg.solve(A * s[:, :, None], (b * s)[:, :, None])[:, :, 0]
+
+    def _helmholtz(self, shift, coef, rhs, im, ik):
+        """(I - coef * (L0 - diag((n+shift)^2/r^2 + kappa^2))) x = rhs for the listed
+        modes; rows 0 and N_r-1 replaced by identity (Dirichlet, L2)."""
+        N_r = self.p.N_r
+        q = ((self.n[im] + shift)[:, None] ** 2 / self.r[None, :] ** 2
+             + self.kappa[ik][:, None] ** 2)                  # [B, N_r]
+        A = np.broadcast_to(np.eye(N_r) - coef * self.L0, (len(im), N_r, N_r)).copy()
+        idx = np.arange(N_r)
+        A[:, idx, idx] += coef * q
+        A[:, 0, :] = 0.0
+        A[:, 0, 0] = 1.0
+        A[:, -1, :] = 0.0
+        A[:, -1, -1] = 1.0
+        return self._solve_rows(A, rhs)
+
+    def _poisson(self, g, im, ik):
+        """P phi = g at interior rows, D1 phi = 0 at the wall rows, with
+        P = Q - diag(n^2/r^2 + kappa^2), Q = (D1 + 1/r) G~ (L4, R9)."""
+        N_r = self.p.N_r
+        q = self.n[im][:, None] ** 2 / self.r[None, :] ** 2 + self.kappa[ik][:, None] ** 2
+        A = np.broadcast_to(self.Q, (len(im), N_r, N_r)).copy()
+        idx = np.arange(N_r)
+        A[:, idx, idx] -= q
+        A[:, 0, :] = self.D1[0]
+        A[:, -1, :] = self.D1[-1]
+        zero = (np.asarray(im) == 0) & (np.asarray(ik) == self.p.K)
+        A[zero] = np.eye(N_r)                                 # O8: mode (0,0) is not projected
+        phi = self._solve_rows(A, g)
+        phi[zero] = 0.0
+        return phi
+
+    def substep(self, state, E, dt, modes=None, chunk=2048):
+        """One implicit sub-step L1..L5 from ``state`` = (ur, ut, uz, T, p) with explicit
+        term E = [E_r, E_theta, E_z, (E_T)].  ``modes``: optional (im, ik) index arrays to
+        restrict to sampled modes (returns arrays [N_r, B]); default all modes."""
+        p = self.p
+        c = p.c
+        ur, ut, uz, T, pr = state
+        N_r = p.N_r
+        full = modes is None
+        if full:
+            IM, IK = np.meshgrid(np.arange(p.M + 1), np.arange(2 * p.K + 1), indexing="ij")
+            IM, IK = IM.ravel(), IK.ravel()
+        else:
+            IM, IK = (np.asarray(x) for x in modes)
+        r = self.r[:, None, None]
+        n = self.n[None, :, None]
+        # L1 right-hand sides, formed for all modes (cheap) then gathered per mode
+        up, um = ur + 1j * ut, ur - 1j * ut
+        Ep, Em = E[0] + 1j * E[1], E[0] - 1j * E[1]
+        dp = self.d_r(pr)
+        rp = up + dt * ((1 - c) * self.lap(up, +1) + Ep - (dp - n / r * pr))
+        rm = um + dt * ((1 - c) * self.lap(um, -1) + Em - (dp + n / r * pr))
+        rz = uz + dt * ((1 - c) * self.lap(uz, 0) + E[2] - 1j * self.kappa[None, None, :] * pr)
+        rhs = [rp, rm, rz]
+        if p.heated:
+            rhs.append(T + dt * ((1 - c) / p.Pr * self.lap(T, 0) + E[3]))
+        # Dirichlet data (R1): u_theta = Re_i, Re_o; u_r = u_z = 0; T = +1/2, -1/2
+        for a in rhs:
+            a[0] = 0.0
+            a[-1] = 0.0
+        rp[0, 0, p.K], rp[-1, 0, p.K] = 1j * p.Re_i, 1j * p.Re_o
+        rm[0, 0, p.K], rm[-1, 0, p.K] = -1j * p.Re_i, -1j * p.Re_o
+        if p.heated:
+            rhs[3][0, 0, p.K], rhs[3][-1, 0, p.K] = 0.5, -0.5
+        nB = len(IM)
+        out = [np.empty((N_r, nB), complex) for _ in range(5)]
+        for s in range(0, nB, chunk):
+            im, ik = IM[s:s + chunk], IK[s:s + chunk]
+            g_ = lambda a: a[:, im, ik].T                    # [B, N_r]
+            # L2 Helmholtz solves
+            ups = self._helmholtz(+1, c * dt, g_(rp), im, ik)
+            ums = self._helmholtz(-1, c * dt, g_(rm), im, ik)
+            uzs = self._helmholtz(0, c * dt, g_(rz), im, ik)
+            Tn = self._helmholtz(0, c * dt / p.Pr, g_(rhs[3]), im, ik) if p.heated else None
+            # L3 recombine + divergence
+            urs = (ups + ums) / 2
+            uts = (ups - ums) / 2j
+            nn, kk, rr = self.n[im][:, None], self.kappa[ik][:, None], self.r[None, :]
+            g = urs @ self.D1.T + urs / rr + 1j * nn / rr * uts + 1j * kk * uzs
+            g[:, 0] = 0.0
+            g[:, -1] = 0.0
+            # L4 pressure Poisson (all modes except (0,0), O8)
+            phi = self._poisson(g, im, ik)
+            zero = (im == 0) & (ik == p.K)
+            # L5 correct + update
+            urn = urs - phi @ self.Gt.T
+            utn = uts - 1j * nn / rr * phi
+            uzn = uzs - 1j * kk * phi
+            urn[zero] = 0.0                                   # O8: u_r(0,0) := 0
+            pn = g_(pr) + phi / dt
+            for o, v in zip(out, (urn, utn, uzn, Tn, pn)):
+                if v is not None:
+                    o[:, s:s + chunk] = v.T
+        if not p.heated:
+            out[3] = None
+        if full:
+            shp = (N_r, p.M + 1, 2 * p.K + 1)
+            out = [None if o is None else o.reshape(shp) for o in out]
+        return out
+
+    # ---------------------------------------------------------------- O7 step
+    def step(self, state, dt):
+        """Predictor-corrector step (R10: c = 1/2, one corrector pass).
+        N0 = N(u^n); u^1 = substep(N0) (its pressure discarded); N1 = N(u^1);
+        u^{n+1} = substep(c N1 + (1-c) N0), both sub-steps starting from (u^n, T^n, p^n)."""
+        c = self.p.c
+        nf = 4 if self.p.heated else 3
+        N0 = self.nonlinear(*state[:nf])
+        s1 = self.substep(state, N0, dt)
+        N1 = self.nonlinear(*s1[:nf])
+        return self.substep(state, [c * a + (1 - c) * b for a, b in zip(N1, N0)], dt)
+
+    # ---------------------------------------------------------------- basic states
+    def zeros(self):
+        p = self.p
+        return np.zeros((p.N_r, p.M + 1, 2 * p.K + 1), complex)
+
+    def base_state_discrete(self):
+        """Discrete basic state: u_theta(r), T(r) (and the buoyancy-driven
+        axial flow w(r), R11) solving the *discrete* steady equations in mode (0,0)."""
+        p = self.p
+        r = self.r
+
+        def solve(L, bi, bo, rhs=None):
+            A = L.copy()
+            A[0] = 0
+            A[0, 0] = 1
+            A[-1] = 0
+            A[-1, -1] = 1
+            b = np.zeros(p.N_r) if rhs is None else rhs.copy()
+            b[0], b[-1] = bi, bo
+            return np.linalg.solve(A, b)
+
+        ur, ut, uz = self.zeros(), self.zeros(), self.zeros()
+        ut[:, 0, p.K] = solve(self.L0 - np.diag(1 / r ** 2), p.Re_i, p.Re_o)
+        T = None
+        if p.heated:
+            T = self.zeros()
+            T[:, 0, p.K] = solve(self.L0, 0.5, -0.5)
+            uz[:, 0, p.K] = solve(self.L0, 0.0, 0.0, -(p.Ra / p.Pr) * T[:, 0, p.K].real)
+        return [ur, ut, uz, T, self.zeros()]
+
+
+def rel_l2(a_list, b_list):
+    """R14 parity norm: ||a - b||_2 / ||b||_2 over the concatenation of all fields."""
+    num = sum(np.linalg.norm((a - b).ravel()) ** 2 for a, b in zip(a_list, b_list) if b is not None)
+    den = sum(np.linalg.norm(b.ravel()) ** 2 for b in b_list if b is not None)
+    return float(np.sqrt(num / den))
