@@ -1,0 +1,128 @@
+/* nsc.h -- C ABI of libnsc.so: one predictor-corrector time step of the nsCouette method
+ * (arxiv/paper_1908_00587) for incompressible, optionally heated Taylor-Couette flow,
+ * computed entirely by hand-written sm_100a CUDA kernels on one B200.
+ *
+ * What the library computes (citations: PAPER.md:<line>; BJ = BASELINE.json north_star;
+ * R# = reading listed in DESIGN.md):
+ *   - Fourier-Galerkin in theta and z, 9-point finite differences on a run-time selectable
+ *     radial grid, axially periodic, cylindrical primitive
+ *     variables u_r, u_theta, u_z, p, (T);
+ *   - the pseudospectral nonlinear term N = -(u.grad)u with the curvature terms, Boussinesq
+ *     buoyancy and -(u.grad)T (BJ (a)), 3/2-rule padded (R4, R5);
+ *   - the implicit predictor-corrector sub-steps: per Fourier mode banded
+ *     Helmholtz solves in u_+- = u_r +- i u_theta, u_z, T and a pressure-Poisson projection
+ *     (BJ (b); "linear terms ... independently per Fourier mode").
+ *
+ * Conventions common to every call
+ *   Spectral field  complex128 (re, im interleaved), shape [N_r][M_theta+1][2 K_z+1], the axial
+ *                   index fastest; entry (j, m, kk) is radial node j (j = 0 inner wall), azimuthal
+ *                   mode m (wavenumber n = m k_theta0), axial mode k = kk - K_z (kappa = k alpha).
+ *   Units           gap d = r_o - r_i = 1, time d^2/nu, velocity nu/d, so Re_i, Re_o
+ *                   are the wall speeds; T = +1/2 at r_i, -1/2 at r_o (R1).
+ *   Pointers        "d_" = DEVICE pointer, "h_" = HOST pointer.  The caller owns every buffer it
+ *                   passes; the library owns the context, its copy of the state and all work space.
+ *   Streams         all device work is enqueued on the stream given to nsc_set_stream (default:
+ *                   the legacy default stream) and is asynchronous; only nsc_create,
+ *                   nsc_destroy and the *_host calls synchronise.
+ *   Errors          0 on success, a negative NSC_E* code otherwise; nsc_last_error() gives text.
+ *                   Nothing throws across the ABI.  There is no CPU fallback: without a CUDA
+ *                   device nsc_create fails with NSC_ECUDA.
+ *   Temperature     enabled iff Ra != 0 (R13); then the T pointers are required, else ignored.
+ */
+#ifndef NSC_H
+#define NSC_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nsc_ctx nsc_ctx;
+
+enum {
+    NSC_OK = 0,
+    NSC_EINVAL = -1,  /* bad argument (sizes, ranges, NULL where a pointer is required)      */
+    NSC_ENOMEM = -2,  /* host or device allocation failed                                       */
+    NSC_ECUDA = -3,   /* a CUDA runtime call or kernel launch failed                            */
+    NSC_ESTATE = -4   /* call out of order (nsc_step / nsc_nonlinear before nsc_set_state)      */
+};
+
+/* Extended creation parameters (nsc_create fills the defaults marked below). */
+typedef struct nsc_params {
+    int N_r;          /* radial nodes, >= 9 (9-point stencil)                      */
+    int M_theta;      /* azimuthal modes m = 0..M_theta; M_theta in {4,8,...,512} (power of two)  */
+    int K_z;          /* axial modes k = -K_z..K_z;     K_z in {4,8,...,512} (power of two)       */
+    double eta;       /* radius ratio r_i / r_o, 0 < eta < 1                                      */
+    double alpha;     /* axial base wavenumber (domain length 2 pi / alpha), > 0                  */
+    int k_theta0;     /* azimuthal base wavenumber, >= 1                                          */
+    double Re_i, Re_o;/* inner / outer wall speed (units nu/d)                                    */
+    double Ra, Pr;    /* Rayleigh, Prandtl number; Ra == 0 switches temperature off; Pr > 0       */
+    int radial_grid;  /* 0 uniform, 1 Chebyshev-Gauss-Lobatto clustering (R2)                     */
+    int n_theta_phys; /* physical grid points in theta; 0 => 3 M_theta (3/2 rule, R4)             */
+    int n_z_phys;     /* physical grid points in z;     0 => 3 K_z; allowed: 3*2^p or 6*2^p lengths
+                         in {12,24,...,1536} that are >= the 3/2 rule                              */
+    double c;         /* implicitness of the linear terms; 0 => 0.5 (R10)                         */
+    int device;       /* CUDA device ordinal; -1 => current device                                */
+    int radial_chunk; /* radial nodes per pass of the transform pipeline; 0 => automatic          */
+} nsc_params;
+
+/* BJ: nsc_create(N_r, M_theta, K_z, eta, alpha, k_theta0, Re_i, Re_o, Ra, Pr, radial-grid type).
+ * Builds the plan on the host in extended precision (radial grid, 9-point weights, operator
+ * band tables, twiddle tables), uploads it and allocates state and work space.  *out is set
+ * only on success.  Synchronises the device. */
+int nsc_create(nsc_ctx** out, int N_r, int M_theta, int K_z, double eta, double alpha, int k_theta0,
+               double Re_i, double Re_o, double Ra, double Pr, int radial_grid);
+int nsc_create_ex(nsc_ctx** out, const nsc_params* p);
+
+/* Frees everything the context owns.  Synchronises.  NULL is a no-op. */
+int nsc_destroy(nsc_ctx* ctx);
+
+/* cudaStream_t (as void*) on which all later work of this context is enqueued. */
+int nsc_set_stream(nsc_ctx* ctx, void* cuda_stream);
+
+/* Radial nodes r_j, j = 0..N_r-1, written to h_r (host, N_r doubles). */
+int nsc_get_grid(const nsc_ctx* ctx, double* h_r);
+
+/* Copies a state into the context (device-to-device on the stream).  d_T required iff Ra != 0;
+ * d_p may be NULL (p = 0).  Each pointer: one spectral field as described above. */
+int nsc_set_state(nsc_ctx* ctx, const void* d_ur, const void* d_uth, const void* d_uz,
+                  const void* d_T, const void* d_p);
+/* Copies the current state out; NULL pointers are skipped. */
+int nsc_get_state(nsc_ctx* ctx, void* d_ur, void* d_uth, void* d_uz, void* d_T, void* d_p);
+/* The same with HOST buffers (pinned or pageable); the host-to-device / device-to-host copies
+ * run on the context's stream and the call returns after they completed. */
+int nsc_set_state_host(nsc_ctx* ctx, const void* h_ur, const void* h_uth, const void* h_uz,
+                       const void* h_T, const void* h_p);
+int nsc_get_state_host(nsc_ctx* ctx, void* h_ur, void* h_uth, void* h_uz, void* h_T, void* h_p);
+
+/* Steps N1-N6 of DESIGN.md (BJ (a)): N(current state), buoyancy included, written to the
+ * caller's device buffers (d_NT required iff Ra != 0); the state is unchanged. */
+int nsc_nonlinear(nsc_ctx* ctx, void* d_Nr, void* d_Nth, void* d_Nz, void* d_NT);
+
+/* Steps L1-L5 (BJ (b)): one implicit sub-step of size dt from the current state with the explicit
+ * term E given by the caller (device buffers, same layout; d_ET required iff Ra != 0):
+ *   Helmholtz solves for u_+-, u_z, (T) -> divergence -> pressure Poisson -> correction;
+ *   the state (u, T, p) is replaced by the result.  Exposed so that the linear stage can be
+ *   checked on its own; nsc_step composes it with nsc_nonlinear internally. */
+int nsc_substep(nsc_ctx* ctx, const void* d_Er, const void* d_Eth, const void* d_Ez,
+                const void* d_ET, double dt);
+
+/* One predictor-corrector step of size dt > 0 (R10: c = 1/2, one corrector pass):
+ *   N0 = N(u^n); u^1 = substep(N0); N1 = N(u^1); u^{n+1} = substep(c N1 + (1-c) N0), both
+ *   sub-steps starting from (u^n, T^n, p^n).  The first call with a new dt factors the
+ *   per-mode banded matrices (kept until dt changes). */
+int nsc_step(nsc_ctx* ctx, double dt);
+
+/* Text of the last error of this context ("" if none); valid until the next call on ctx.
+ * With ctx == NULL: the text of the last failed nsc_create on this thread. */
+const char* nsc_last_error(const nsc_ctx* ctx);
+
+/* Bytes of device memory the context holds (state + work + factors), for reports. */
+long long nsc_device_bytes(const nsc_ctx* ctx);
+
+/* Number of kernel launches this context has enqueued so far (for bench.py's gpu_launches). */
+long long nsc_launch_count(const nsc_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NSC_H */

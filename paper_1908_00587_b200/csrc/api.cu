@@ -1,0 +1,256 @@
+// api.cu -- the C ABI of include/nsc.h: argument checks, allocation, and the composition of
+// one predictor-corrector step (O7) from the kernels of nonlinear.cu
+// and linear.cu.  No arithmetic of the method happens on the host after nsc_create.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "nsc_internal.h"
+
+namespace nsc {
+
+bool fft_length_supported(int n);
+
+static thread_local std::string g_create_err;
+
+int fail(nsc_ctx* c, int code, const std::string& msg) {
+    if (c)
+        c->err = msg;
+    else
+        g_create_err = msg;
+    return code;
+}
+
+int cuda_fail(nsc_ctx* c, cudaError_t e, const char* what) {
+    std::string m = std::string(what) + ": " + cudaGetErrorString(e);
+    fail(c, NSC_ECUDA, m);
+    return e == cudaErrorMemoryAllocation ? NSC_ENOMEM : NSC_ECUDA;
+}
+
+static int dev_alloc(nsc_ctx* c, cd** dst, size_t elems, bool zero) {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, elems * sizeof(cd));
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc(field)");
+    c->allocs.push_back(p);
+    c->dev_bytes += (long long)(elems * sizeof(cd));
+    if (zero) {
+        e = cudaMemset(p, 0, elems * sizeof(cd));
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemset(field)");
+    }
+    *dst = (cd*)p;
+    return NSC_OK;
+}
+
+static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
+
+}  // namespace nsc
+
+using namespace nsc;
+
+extern "C" {
+
+int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
+    if (!out || !pp) return fail(nullptr, NSC_EINVAL, "nsc_create: NULL argument");
+    nsc_params p = *pp;
+    if (p.N_r < NPT) return fail(nullptr, NSC_EINVAL, "nsc_create: N_r must be >= 9");
+    if (!pow2_in(p.M_theta, 4, 512) || !pow2_in(p.K_z, 4, 512))
+        return fail(nullptr, NSC_EINVAL, "nsc_create: M_theta and K_z must be powers of two in [4, 512]");
+    if (!(p.eta > 0.0 && p.eta < 1.0)) return fail(nullptr, NSC_EINVAL, "nsc_create: eta must be in (0, 1)");
+    if (!(p.alpha > 0.0)) return fail(nullptr, NSC_EINVAL, "nsc_create: alpha must be > 0");
+    if (p.k_theta0 < 1) return fail(nullptr, NSC_EINVAL, "nsc_create: k_theta0 must be >= 1");
+    if (p.Ra != 0.0 && !(p.Pr > 0.0)) return fail(nullptr, NSC_EINVAL, "nsc_create: Pr must be > 0 when Ra != 0");
+    if (p.radial_grid != 0 && p.radial_grid != 1) return fail(nullptr, NSC_EINVAL, "nsc_create: radial_grid must be 0 or 1");
+    if (p.n_theta_phys == 0) p.n_theta_phys = 3 * p.M_theta;
+    if (p.n_z_phys == 0) p.n_z_phys = 3 * p.K_z;
+    if (p.n_theta_phys < 3 * p.M_theta || p.n_z_phys < 3 * p.K_z || !fft_length_supported(p.n_theta_phys) ||
+        !fft_length_supported(p.n_z_phys))
+        return fail(nullptr, NSC_EINVAL, "nsc_create: unsupported physical grid size");
+    if (p.c == 0.0) p.c = 0.5;
+    if (!(p.c > 0.0 && p.c <= 1.0)) return fail(nullptr, NSC_EINVAL, "nsc_create: c must be in (0, 1]");
+    if (p.Ra == 0.0) p.Pr = 1.0;
+
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, NSC_ECUDA, "nsc_create: no CUDA device (there is no CPU fallback)");
+    }
+    if (p.device >= 0) {
+        e = cudaSetDevice(p.device);
+        if (e != cudaSuccess) return fail(nullptr, NSC_ECUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
+    }
+    nsc_ctx* c = new (std::nothrow) nsc_ctx();
+    if (!c) return fail(nullptr, NSC_ENOMEM, "nsc_create: out of host memory");
+    c->p = p;
+    c->N_r = p.N_r;
+    c->M = p.M_theta;
+    c->K = p.K_z;
+    c->M1 = c->M + 1;
+    c->NK = 2 * c->K + 1;
+    c->MP = (c->M1 + 7) / 8 * 8;
+    c->Nt = p.n_theta_phys;
+    c->Nz = p.n_z_phys;
+    c->heated = p.Ra != 0.0;
+    c->nf = c->heated ? 4 : 3;
+    c->F = (size_t)c->N_r * c->M1 * c->NK;
+    c->P = c->M1 * (c->K + 1);
+    // radial chunk of the transform pipeline: work arrays of ~2 GiB unless told otherwise
+    const size_t per_level = (size_t)4 * c->nf * c->Nz * c->MP * sizeof(cd);
+    int jc = p.radial_chunk > 0 ? p.radial_chunk : (int)(((size_t)2 << 30) / per_level);
+    if (jc < 1) jc = 1;
+    if (jc > c->N_r) jc = c->N_r;
+    c->JC = jc;
+
+    int rc = build_plan(c);
+    if (!rc) {
+        for (int i = 0; i < 5 && !rc; ++i)
+            if (i != 3 || c->heated) rc = dev_alloc(c, &c->state[i], c->F, true);
+        for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->W[i], c->F, false);
+        for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->N0[i], c->F, false);
+        for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->N1[i], c->F, false);
+        if (!rc) rc = dev_alloc(c, &c->G, c->F, false);
+        if (!rc) rc = dev_alloc(c, &c->zbuf, (size_t)3 * c->nf * c->JC * c->Nz * c->MP, true);
+        if (!rc) rc = dev_alloc(c, &c->tbuf, (size_t)c->nf * c->JC * c->Nz * c->MP, true);
+    }
+    if (!rc) {
+        e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) rc = cuda_fail(c, e, "nsc_create: cudaDeviceSynchronize");
+    }
+    if (rc) {
+        g_create_err = c->err;
+        nsc_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return NSC_OK;
+}
+
+int nsc_create(nsc_ctx** out, int N_r, int M_theta, int K_z, double eta, double alpha, int k_theta0, double Re_i,
+               double Re_o, double Ra, double Pr, int radial_grid) {
+    nsc_params p;
+    memset(&p, 0, sizeof(p));
+    p.N_r = N_r;
+    p.M_theta = M_theta;
+    p.K_z = K_z;
+    p.eta = eta;
+    p.alpha = alpha;
+    p.k_theta0 = k_theta0;
+    p.Re_i = Re_i;
+    p.Re_o = Re_o;
+    p.Ra = Ra;
+    p.Pr = Pr;
+    p.radial_grid = radial_grid;
+    p.device = -1;
+    return nsc_create_ex(out, &p);
+}
+
+int nsc_destroy(nsc_ctx* c) {
+    if (!c) return NSC_OK;
+    cudaDeviceSynchronize();
+    for (void* p : c->allocs) cudaFree(p);
+    cudaGetLastError();
+    delete c;
+    return NSC_OK;
+}
+
+int nsc_set_stream(nsc_ctx* c, void* s) {
+    if (!c) return NSC_EINVAL;
+    c->stream = (cudaStream_t)s;
+    return NSC_OK;
+}
+
+int nsc_get_grid(const nsc_ctx* c, double* h_r) {
+    if (!c || !h_r) return NSC_EINVAL;
+    memcpy(h_r, c->r.data(), sizeof(double) * c->N_r);
+    return NSC_OK;
+}
+
+static int copy_state(nsc_ctx* c, const void* const* src, void* const* dst, cudaMemcpyKind kind, bool set) {
+    for (int i = 0; i < 5; ++i) {
+        if (i == 3 && !c->heated) continue;
+        const size_t bytes = c->F * sizeof(cd);
+        if (set) {
+            if (src[i])
+                NSC_CUDA(c, cudaMemcpyAsync(c->state[i], src[i], bytes, kind, c->stream));
+            else if (i == 4)
+                NSC_CUDA(c, cudaMemsetAsync(c->state[4], 0, bytes, c->stream));
+            else
+                return fail(c, NSC_EINVAL, "nsc_set_state: required field pointer is NULL");
+        } else if (dst[i]) {
+            NSC_CUDA(c, cudaMemcpyAsync(dst[i], c->state[i], bytes, kind, c->stream));
+        }
+    }
+    return NSC_OK;
+}
+
+int nsc_set_state(nsc_ctx* c, const void* ur, const void* uth, const void* uz, const void* T, const void* p) {
+    if (!c) return NSC_EINVAL;
+    const void* src[5] = {ur, uth, uz, T, p};
+    int rc = copy_state(c, src, nullptr, cudaMemcpyDeviceToDevice, true);
+    if (!rc) c->have_state = true;
+    return rc;
+}
+
+int nsc_get_state(nsc_ctx* c, void* ur, void* uth, void* uz, void* T, void* p) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_get_state before nsc_set_state");
+    void* dst[5] = {ur, uth, uz, T, p};
+    return copy_state(c, nullptr, dst, cudaMemcpyDeviceToDevice, false);
+}
+
+int nsc_set_state_host(nsc_ctx* c, const void* ur, const void* uth, const void* uz, const void* T, const void* p) {
+    if (!c) return NSC_EINVAL;
+    const void* src[5] = {ur, uth, uz, T, p};
+    int rc = copy_state(c, src, nullptr, cudaMemcpyHostToDevice, true);
+    if (rc) return rc;
+    NSC_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_state = true;
+    return NSC_OK;
+}
+
+int nsc_get_state_host(nsc_ctx* c, void* ur, void* uth, void* uz, void* T, void* p) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_get_state_host before nsc_set_state");
+    void* dst[5] = {ur, uth, uz, T, p};
+    int rc = copy_state(c, nullptr, dst, cudaMemcpyDeviceToHost, false);
+    if (rc) return rc;
+    NSC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NSC_OK;
+}
+
+int nsc_nonlinear(nsc_ctx* c, void* Nr, void* Nth, void* Nz, void* NT) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_nonlinear before nsc_set_state");
+    if (!Nr || !Nth || !Nz || (c->heated && !NT)) return fail(c, NSC_EINVAL, "nsc_nonlinear: NULL output pointer");
+    cd* out[MAXF] = {(cd*)Nr, (cd*)Nth, (cd*)Nz, (cd*)NT};
+    return launch_nonlinear(c, c->state, out);
+}
+
+int nsc_substep(nsc_ctx* c, const void* Er, const void* Eth, const void* Ez, const void* ET, double dt) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_substep before nsc_set_state");
+    if (!(dt > 0.0)) return fail(c, NSC_EINVAL, "nsc_substep: dt must be > 0");
+    if (!Er || !Eth || !Ez || (c->heated && !ET)) return fail(c, NSC_EINVAL, "nsc_substep: NULL explicit-term pointer");
+    cd* E[MAXF] = {(cd*)Er, (cd*)Eth, (cd*)Ez, (cd*)ET};
+    return launch_substep(c, E, 1.0, nullptr, 0.0, dt, c->state, c->state[4]);
+}
+
+int nsc_step(nsc_ctx* c, double dt) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_step before nsc_set_state");
+    if (!(dt > 0.0)) return fail(c, NSC_EINVAL, "nsc_step: dt must be > 0");
+    int rc;
+    // N0 = N(u^n);  u^1 = substep(N0) -> W (its pressure is discarded)
+    if ((rc = launch_nonlinear(c, c->state, c->N0))) return rc;
+    if ((rc = launch_substep(c, c->N0, 1.0, nullptr, 0.0, dt, c->W, nullptr))) return rc;
+    // N1 = N(u^1);  u^{n+1} = substep(c N1 + (1 - c) N0) from (u^n, p^n), in place
+    if ((rc = launch_nonlinear(c, c->W, c->N1))) return rc;
+    return launch_substep(c, c->N1, c->p.c, c->N0, 1.0 - c->p.c, dt, c->state, c->state[4]);
+}
+
+const char* nsc_last_error(const nsc_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+long long nsc_device_bytes(const nsc_ctx* c) { return c ? c->dev_bytes : 0; }
+
+long long nsc_launch_count(const nsc_ctx* c) { return c ? c->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,488 @@
+// linear.cu -- the implicit sub-step (DESIGN.md steps L1-L5; BASELINE.json north_star (b)):
+//   L1 right-hand sides, L2 banded Helmholtz solves for u_+- = u_r +- i u_theta, u_z, T,
+//   L3 recombination + divergence, L4 pressure-Poisson solve, L5 correction and update.
+// PAPER.md:46 (predictor-corrector, implicit linear terms), PAPER.md:64 ("linear terms ...
+// independently per Fourier mode").
+//
+// Per-mode matrices differ from mode to mode only on the diagonal:
+//   Helmholtz  A = I - coef (L0 - diag((n + shift)^2 / r^2 + kappa^2)),  identity rows at the walls
+//   Poisson    P = Q - diag(n^2 / r^2 + kappa^2),  Neumann rows D1[wall] at the walls (R9)
+// and are the same for +k and -k, so one thread serves the pair (m, |k|).  They are LU-factored
+// without pivoting inside their row envelope (no fill-in outside it) once per dt (Helmholtz) /
+// once per context (Poisson); the solves stream the factors with pair-major (coalesced) access.
+#include "nsc_internal.h"
+
+namespace nsc {
+
+// ------------------------------------------------------------------------------------------
+// factorisation (set-up; generic, one thread per pair, row scratch in local memory)
+struct FacArgs {
+    const double* band;   // [N_r][BW] operator rows (L0 or Q)
+    const int* bcol0;     // [N_r] first column of the stored row
+    const double* D1;     // wall rows of the Poisson matrix
+    const int* s0;
+    const double* rinv;
+    const double* nm;
+    const double* kap;
+    const int *lo, *hi, *offL, *offU;
+    double* L;
+    double* U;
+    int N_r, K, P, bw;
+    int kind;             // 0 Helmholtz, 1 Poisson
+    double coef, shift;
+};
+
+constexpr int ROWMAX = 32;
+
+__global__ void k_factor(FacArgs a) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= a.P) return;
+    const int m = p / (a.K + 1), ka = p % (a.K + 1);
+    const double n = a.nm[m] + a.shift;
+    const double kap = a.kap[a.K + ka];
+    const size_t P = a.P;
+    const bool singular = (a.kind == 1 && m == 0 && ka == 0);   // O8: mode (0,0) is not projected
+    double w[ROWMAX];
+    for (int j = 0; j < a.N_r; ++j) {
+        const int lo = a.lo[j], hi = a.hi[j];
+        const int width = hi - lo + 1;
+        for (int i = 0; i < width; ++i) w[i] = 0.0;
+        const bool wall = (j == 0 || j == a.N_r - 1);
+        const double ri = a.rinv[j];
+        const double q = n * n * ri * ri + kap * kap;
+        if (a.kind == 0) {
+            if (wall) {
+                w[j - lo] = 1.0;
+            } else {
+                const int c0 = a.bcol0[j];
+                for (int l = 0; l < a.bw; ++l) w[c0 + l - lo] = -a.coef * a.band[j * a.bw + l];
+                w[j - lo] += 1.0 + a.coef * q;
+            }
+        } else {
+            if (wall) {
+                const int c0 = a.s0[j];
+                for (int l = 0; l < NPT; ++l) w[c0 + l - lo] = a.D1[j * NPT + l];
+            } else {
+                const int c0 = a.bcol0[j];
+                for (int l = 0; l < a.bw; ++l) {
+                    const int col = c0 + l;
+                    if (col <= hi) w[col - lo] = a.band[j * a.bw + l];
+                }
+                w[j - lo] -= q;
+            }
+        }
+        // eliminate columns lo..j-1 with the already factored rows
+        for (int cidx = lo; cidx < j; ++cidx) {
+            const size_t ou = (size_t)a.offU[cidx];
+            const double l = w[cidx - lo] * a.U[ou * P + p];          // times 1/pivot of row cidx
+            a.L[((size_t)a.offL[j] + (cidx - lo)) * P + p] = singular ? 0.0 : l;
+            const int nu = a.hi[cidx] - cidx;
+            for (int i = 1; i <= nu; ++i) w[cidx + i - lo] -= l * a.U[(ou + i) * P + p];
+        }
+        const size_t ou = (size_t)a.offU[j];
+        a.U[ou * P + p] = singular ? 0.0 : 1.0 / w[j - lo];
+        for (int i = 1; i <= hi - j; ++i) a.U[(ou + i) * P + p] = singular ? 0.0 : w[j + i - lo];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// banded solve, in place, both modes (m, +k) and (m, -k) of a pair per thread
+struct SolveArgs {
+    const double* L;
+    const double* U;
+    const int *lo, *hi, *offL, *offU;
+    cd* x;              // [N_r][M1][NK]
+    int N_r, M1, NK, K, P;
+};
+
+template <int WREG, int WMAX>
+__global__ void __launch_bounds__(128) k_band_solve(SolveArgs a) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= a.P) return;
+    const int m = p / (a.K + 1), ka = p % (a.K + 1);
+    const size_t P = a.P;
+    const size_t plane = (size_t)a.M1 * a.NK;
+    cd* xp = a.x + (size_t)m * a.NK + a.K + ka;
+    cd* xm = a.x + (size_t)m * a.NK + a.K - ka;
+    cd wp[WMAX], wm[WMAX];                      // w[WMAX-1] = most recent row
+#pragma unroll
+    for (int i = 0; i < WMAX; ++i) wp[i] = wm[i] = mk(0.0, 0.0);
+    // forward: y_j = b_j - sum_i L[j][i] y_{lo+i}
+    for (int j = 0; j < a.N_r; ++j) {
+        const int nl = j - a.lo[j];
+        const double* Lr = a.L + (size_t)a.offL[j] * P + p;
+        cd bp = xp[(size_t)j * plane], bm = xm[(size_t)j * plane];
+        if (nl == WREG) {
+#pragma unroll
+            for (int q = WMAX - WREG; q < WMAX; ++q) {
+                const double l = Lr[(size_t)(q - (WMAX - WREG)) * P];
+                bp.x = fma(-l, wp[q].x, bp.x);
+                bp.y = fma(-l, wp[q].y, bp.y);
+                bm.x = fma(-l, wm[q].x, bm.x);
+                bm.y = fma(-l, wm[q].y, bm.y);
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < WMAX; ++q) {
+                const int i = q - (WMAX - nl);
+                if (i >= 0) {
+                    const double l = Lr[(size_t)i * P];
+                    bp.x = fma(-l, wp[q].x, bp.x);
+                    bp.y = fma(-l, wp[q].y, bp.y);
+                    bm.x = fma(-l, wm[q].x, bm.x);
+                    bm.y = fma(-l, wm[q].y, bm.y);
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < WMAX - 1; ++q) {
+            wp[q] = wp[q + 1];
+            wm[q] = wm[q + 1];
+        }
+        wp[WMAX - 1] = bp;
+        wm[WMAX - 1] = bm;
+        xp[(size_t)j * plane] = bp;
+        if (ka != 0) xm[(size_t)j * plane] = bm;
+    }
+    // backward: x_j = (y_j - sum_{i>=1} U[j][i] x_{j+i}) / pivot;  w[0] = x_{j+1}
+    for (int j = a.N_r - 1; j >= 0; --j) {
+        const int nu = a.hi[j] - j;
+        const double* Ur = a.U + (size_t)a.offU[j] * P + p;
+        cd yp = xp[(size_t)j * plane], ym = xm[(size_t)j * plane];
+        if (nu == WREG) {
+#pragma unroll
+            for (int q = 0; q < WREG; ++q) {
+                const double u = Ur[(size_t)(q + 1) * P];
+                yp.x = fma(-u, wp[q].x, yp.x);
+                yp.y = fma(-u, wp[q].y, yp.y);
+                ym.x = fma(-u, wm[q].x, ym.x);
+                ym.y = fma(-u, wm[q].y, ym.y);
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < WMAX; ++q) {
+                if (q < nu) {
+                    const double u = Ur[(size_t)(q + 1) * P];
+                    yp.x = fma(-u, wp[q].x, yp.x);
+                    yp.y = fma(-u, wp[q].y, yp.y);
+                    ym.x = fma(-u, wm[q].x, ym.x);
+                    ym.y = fma(-u, wm[q].y, ym.y);
+                }
+            }
+        }
+        const double dinv = Ur[0];
+        yp = dinv * yp;
+        ym = dinv * ym;
+#pragma unroll
+        for (int q = WMAX - 1; q > 0; --q) {
+            wp[q] = wp[q - 1];
+            wm[q] = wm[q - 1];
+        }
+        wp[0] = yp;
+        wm[0] = ym;
+        xp[(size_t)j * plane] = yp;
+        if (ka != 0) xm[(size_t)j * plane] = ym;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// element-wise / stencil kernels
+struct LinArgs {
+    const cd* u[MAXF];     // state n: u_r, u_theta, u_z, T
+    const cd* p;           // pressure n
+    const cd* E0[MAXF];
+    const cd* E1[MAXF];    // may be null
+    cd* W[MAXF];           // work: rhs_+ / rhs_- / rhs_z / rhs_T  ->  u_r*, u_theta*, u_z*, T
+    cd* G;                 // divergence / phi
+    cd* dst[MAXF];         // corrected fields
+    cd* p_dst;             // new pressure (may be null)
+    const double *D1, *L0, *rinv, *nm, *kap;
+    const int* s0;
+    int N_r, M1, NK, K, nf;
+    double dt, c, w0, w1, inv_Pr, Re_i, Re_o;
+};
+
+// L1: rhs_+- = u_+- + dt[(1-c) L_+- u_+- + E_+- - (D1 p -+ (n/r) p)],  rhs_z, rhs_T likewise;
+// wall rows carry the Dirichlet data (R1).
+__global__ void __launch_bounds__(128) k_rhs(LinArgs a) {
+    const int plane = a.M1 * a.NK;
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= plane) return;
+    const int j = blockIdx.y;
+    const int m = e / a.NK, kk = e % a.NK;
+    const size_t o = (size_t)j * plane + e;
+    const bool heated = a.nf == 4;
+    if (j == 0 || j == a.N_r - 1) {
+        const bool m00 = (m == 0 && kk == a.K);
+        const double v = m00 ? (j == 0 ? a.Re_i : a.Re_o) : 0.0;
+        a.W[0][o] = mk(0.0, v);                 // u_+ = u_r + i u_theta = i Re
+        a.W[1][o] = mk(0.0, -v);
+        a.W[2][o] = mk(0.0, 0.0);
+        if (heated) a.W[3][o] = mk(m00 ? (j == 0 ? 0.5 : -0.5) : 0.0, 0.0);
+        return;
+    }
+    const int s = a.s0[j];
+    cd Sr = mk(0, 0), St = mk(0, 0), Sz = mk(0, 0), ST = mk(0, 0), Dp = mk(0, 0);
+#pragma unroll
+    for (int l = 0; l < NPT; ++l) {
+        const size_t ol = (size_t)(s + l) * plane + e;
+        const double wl = a.L0[j * NPT + l], wd = a.D1[j * NPT + l];
+        cd v = a.u[0][ol];
+        Sr.x = fma(wl, v.x, Sr.x);
+        Sr.y = fma(wl, v.y, Sr.y);
+        v = a.u[1][ol];
+        St.x = fma(wl, v.x, St.x);
+        St.y = fma(wl, v.y, St.y);
+        v = a.u[2][ol];
+        Sz.x = fma(wl, v.x, Sz.x);
+        Sz.y = fma(wl, v.y, Sz.y);
+        if (heated) {
+            v = a.u[3][ol];
+            ST.x = fma(wl, v.x, ST.x);
+            ST.y = fma(wl, v.y, ST.y);
+        }
+        v = a.p[ol];
+        Dp.x = fma(wd, v.x, Dp.x);
+        Dp.y = fma(wd, v.y, Dp.y);
+    }
+    const double ri = a.rinv[j], n = a.nm[m], kap = a.kap[kk];
+    const double k2 = kap * kap, r2 = ri * ri;
+    const double qp = (n + 1) * (n + 1) * r2 + k2, qm = (n - 1) * (n - 1) * r2 + k2, q0 = n * n * r2 + k2;
+    const cd ur = a.u[0][o], ut = a.u[1][o], uz = a.u[2][o], pr = a.p[o];
+    cd Er = a.w0 * a.E0[0][o], Et = a.w0 * a.E0[1][o], Ez = a.w0 * a.E0[2][o];
+    if (a.E1[0]) {
+        Er = Er + a.w1 * a.E1[0][o];
+        Et = Et + a.w1 * a.E1[1][o];
+        Ez = Ez + a.w1 * a.E1[2][o];
+    }
+    const double omc = 1.0 - a.c, dt = a.dt;
+    const cd up = ur + mul_i(ut), um = ur - mul_i(ut);
+    const cd Lp = (Sr + mul_i(St)) - qp * up, Lm = (Sr - mul_i(St)) - qm * um;
+    const cd npr = (n * ri) * pr;
+    a.W[0][o] = up + dt * (omc * Lp + (Er + mul_i(Et)) - (Dp - npr));
+    a.W[1][o] = um + dt * (omc * Lm + (Er - mul_i(Et)) - (Dp + npr));
+    a.W[2][o] = uz + dt * (omc * (Sz - q0 * uz) + Ez - kap * mul_i(pr));
+    if (heated) {
+        const cd T = a.u[3][o];
+        cd ET = a.w0 * a.E0[3][o];
+        if (a.E1[3]) ET = ET + a.w1 * a.E1[3][o];
+        a.W[3][o] = T + dt * ((omc * a.inv_Pr) * (ST - q0 * T) + ET);
+    }
+}
+
+// L3a: u_r* = (u_+ + u_-)/2, u_theta* = (u_+ - u_-)/(2i), in place in W[0], W[1]
+__global__ void __launch_bounds__(256) k_recombine(LinArgs a, size_t total) {
+    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= total) return;
+    const cd up = a.W[0][o], um = a.W[1][o];
+    a.W[0][o] = 0.5 * (up + um);
+    a.W[1][o] = 0.5 * mul_mi(up - um);
+}
+
+// L3b: g = D1 u_r* + u_r*/r + (i n / r) u_theta* + i kappa u_z*;  g = 0 in the wall rows
+__global__ void __launch_bounds__(128) k_div(LinArgs a) {
+    const int plane = a.M1 * a.NK;
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= plane) return;
+    const int j = blockIdx.y;
+    const size_t o = (size_t)j * plane + e;
+    if (j == 0 || j == a.N_r - 1) {
+        a.G[o] = mk(0.0, 0.0);
+        return;
+    }
+    const int m = e / a.NK, kk = e % a.NK;
+    const int s = a.s0[j];
+    cd d = mk(0, 0);
+#pragma unroll
+    for (int l = 0; l < NPT; ++l) {
+        const double wd = a.D1[j * NPT + l];
+        const cd v = a.W[0][(size_t)(s + l) * plane + e];
+        d.x = fma(wd, v.x, d.x);
+        d.y = fma(wd, v.y, d.y);
+    }
+    const double ri = a.rinv[j];
+    a.G[o] = d + ri * a.W[0][o] + (a.nm[m] * ri) * mul_i(a.W[1][o]) + a.kap[kk] * mul_i(a.W[2][o]);
+}
+
+// L5: u = u* - (G~ phi, (i n / r) phi, i kappa phi);  p_new = p + phi / dt;  u_r(0,0) := 0 (O8)
+__global__ void __launch_bounds__(128) k_correct(LinArgs a) {
+    const int plane = a.M1 * a.NK;
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= plane) return;
+    const int j = blockIdx.y;
+    const size_t o = (size_t)j * plane + e;
+    const int m = e / a.NK, kk = e % a.NK;
+    cd gphi = mk(0, 0);
+    if (j != 0 && j != a.N_r - 1) {
+        const int s = a.s0[j];
+#pragma unroll
+        for (int l = 0; l < NPT; ++l) {
+            const double wd = a.D1[j * NPT + l];
+            const cd v = a.G[(size_t)(s + l) * plane + e];
+            gphi.x = fma(wd, v.x, gphi.x);
+            gphi.y = fma(wd, v.y, gphi.y);
+        }
+    }
+    const cd phi = a.G[o];
+    const double ri = a.rinv[j];
+    cd ur = a.W[0][o] - gphi;
+    if (m == 0 && kk == a.K) ur = mk(0.0, 0.0);
+    a.dst[0][o] = ur;
+    a.dst[1][o] = a.W[1][o] - (a.nm[m] * ri) * mul_i(phi);
+    a.dst[2][o] = a.W[2][o] - a.kap[kk] * mul_i(phi);
+    if (a.nf == 4 && a.dst[3] != a.W[3]) a.dst[3][o] = a.W[3][o];
+    if (a.p_dst) a.p_dst[o] = a.p[o] + (1.0 / a.dt) * phi;
+}
+
+// ------------------------------------------------------------------------------------------
+static int alloc_factors(nsc_ctx* c, BandFactors& f, const BandShape& s) {
+    if (f.L) return NSC_OK;
+    f.nL = s.nL;
+    f.nU = s.nU;
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, sizeof(double) * (s.nL ? s.nL : 1) * c->P);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc(L factors)");
+    c->allocs.push_back(p);
+    f.L = (double*)p;
+    e = cudaMalloc(&p, sizeof(double) * s.nU * c->P);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc(U factors)");
+    c->allocs.push_back(p);
+    f.U = (double*)p;
+    c->dev_bytes += (long long)(sizeof(double) * (s.nL + s.nU) * c->P);
+    return NSC_OK;
+}
+
+static int run_factor(nsc_ctx* c, BandFactors& f, const BandShape& s, int kind, double coef, double shift) {
+    int rc = alloc_factors(c, f, s);
+    if (rc) return rc;
+    FacArgs a{};
+    a.band = kind == 0 ? c->t.L0 : c->t.Q;
+    a.bcol0 = kind == 0 ? c->t.s0 : c->t.q0;
+    a.bw = kind == 0 ? NPT : QW;
+    a.D1 = c->t.D1;
+    a.s0 = c->t.s0;
+    a.rinv = c->t.rinv;
+    a.nm = c->t.nm;
+    a.kap = c->t.kap;
+    a.lo = s.lo;
+    a.hi = s.hi;
+    a.offL = s.offL;
+    a.offU = s.offU;
+    a.L = f.L;
+    a.U = f.U;
+    a.N_r = c->N_r;
+    a.K = c->K;
+    a.P = c->P;
+    a.kind = kind;
+    a.coef = coef;
+    a.shift = shift;
+    k_factor<<<(c->P + 63) / 64, 64, 0, c->stream>>>(a);
+    c->launches += 1;
+    NSC_CUDA(c, cudaGetLastError());
+    return NSC_OK;
+}
+
+int ensure_factors(nsc_ctx* c, double dt) {
+    int rc;
+    if (!c->facP_ready) {
+        if ((rc = run_factor(c, c->facP, c->shP, 1, 0.0, 0.0))) return rc;
+        c->facP_ready = true;
+    }
+    if (c->fac_dt != dt) {
+        const double coef = c->p.c * dt;
+        if ((rc = run_factor(c, c->facH[0], c->shH, 0, coef, +1.0))) return rc;
+        if ((rc = run_factor(c, c->facH[1], c->shH, 0, coef, -1.0))) return rc;
+        if ((rc = run_factor(c, c->facH[2], c->shH, 0, coef, 0.0))) return rc;
+        if (c->heated) {
+            if (c->p.Pr == 1.0) {
+                c->facT_shared = true;
+            } else {
+                c->facT_shared = false;
+                if ((rc = run_factor(c, c->facH[3], c->shH, 0, coef / c->p.Pr, 0.0))) return rc;
+            }
+        }
+        c->fac_dt = dt;
+    }
+    return NSC_OK;
+}
+
+static int run_solve(nsc_ctx* c, const BandFactors& f, const BandShape& s, cd* x, bool poisson) {
+    SolveArgs a{};
+    a.L = f.L;
+    a.U = f.U;
+    a.lo = s.lo;
+    a.hi = s.hi;
+    a.offL = s.offL;
+    a.offU = s.offU;
+    a.x = x;
+    a.N_r = c->N_r;
+    a.M1 = c->M1;
+    a.NK = c->NK;
+    a.K = c->K;
+    a.P = c->P;
+    const int threads = 128;
+    const int blocks = (c->P + threads - 1) / threads;
+    if (poisson)
+        k_band_solve<8, 12><<<blocks, threads, 0, c->stream>>>(a);
+    else
+        k_band_solve<4, 8><<<blocks, threads, 0, c->stream>>>(a);
+    c->launches += 1;
+    NSC_CUDA(c, cudaGetLastError());
+    return NSC_OK;
+}
+
+int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w1, double dt, cd* const* dst,
+                   cd* p_dst) {
+    int rc = ensure_factors(c, dt);
+    if (rc) return rc;
+    LinArgs a{};
+    for (int i = 0; i < c->nf; ++i) {
+        a.u[i] = c->state[i];
+        a.E0[i] = E0[i];
+        a.E1[i] = E1 ? E1[i] : nullptr;
+        a.W[i] = c->W[i];
+        a.dst[i] = dst[i];
+    }
+    a.p = c->state[4];
+    a.G = c->G;
+    a.p_dst = p_dst;
+    a.D1 = c->t.D1;
+    a.L0 = c->t.L0;
+    a.rinv = c->t.rinv;
+    a.nm = c->t.nm;
+    a.kap = c->t.kap;
+    a.s0 = c->t.s0;
+    a.N_r = c->N_r;
+    a.M1 = c->M1;
+    a.NK = c->NK;
+    a.K = c->K;
+    a.nf = c->nf;
+    a.dt = dt;
+    a.c = c->p.c;
+    a.w0 = w0;
+    a.w1 = w1;
+    a.inv_Pr = 1.0 / c->p.Pr;
+    a.Re_i = c->p.Re_i;
+    a.Re_o = c->p.Re_o;
+    const int plane = c->M1 * c->NK;
+    dim3 gridp((plane + 127) / 128, c->N_r);
+    k_rhs<<<gridp, 128, 0, c->stream>>>(a);
+    c->launches += 1;
+    NSC_CUDA(c, cudaGetLastError());
+    if ((rc = run_solve(c, c->facH[0], c->shH, c->W[0], false))) return rc;
+    if ((rc = run_solve(c, c->facH[1], c->shH, c->W[1], false))) return rc;
+    if ((rc = run_solve(c, c->facH[2], c->shH, c->W[2], false))) return rc;
+    if (c->heated)
+        if ((rc = run_solve(c, c->facT_shared ? c->facH[2] : c->facH[3], c->shH, c->W[3], false))) return rc;
+    k_recombine<<<(unsigned)((c->F + 255) / 256), 256, 0, c->stream>>>(a, c->F);
+    k_div<<<gridp, 128, 0, c->stream>>>(a);
+    c->launches += 2;
+    NSC_CUDA(c, cudaGetLastError());
+    if ((rc = run_solve(c, c->facP, c->shP, c->G, true))) return rc;
+    k_correct<<<gridp, 128, 0, c->stream>>>(a);
+    c->launches += 1;
+    NSC_CUDA(c, cudaGetLastError());
+    return NSC_OK;
+}
+
+}  // namespace nsc

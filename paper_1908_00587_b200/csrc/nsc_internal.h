@@ -1,0 +1,103 @@
+// nsc_internal.h -- context, device tables and kernel-launcher prototypes shared by the
+// translation units of libnsc.so.  Not part of the ABI (that is include/nsc.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <string>
+#include <vector>
+#include "../../include/nsc.h"
+#include "fft.cuh"
+
+namespace nsc {
+
+constexpr int NPT = 9;        // finite-difference stencil length (default nine points)
+constexpr int QW = 17;        // stored width of a Poisson-operator row, Q = (D1 + 1/r) G~
+constexpr int MAXF = 4;       // u_r, u_theta, u_z, T
+
+// Variable-band LU factors of one family of per-mode matrices, pair-major ("pair" = (m, |k|)):
+// entry e of row j of pair p lives at  L[(offL[j] + e) * P + p],  U[(offU[j] + e) * P + p];
+// U row = [1/pivot, upper entries...].
+struct BandFactors {
+    double* L = nullptr;
+    double* U = nullptr;
+    size_t nL = 0, nU = 0;    // entries per pair
+};
+
+// Row envelope of a banded matrix family: columns lo[j]..hi[j]; nl = j - lo, nu = hi - j.
+struct BandShape {
+    int* lo = nullptr;        // device [N_r]
+    int* hi = nullptr;
+    int* offL = nullptr;      // device [N_r] prefix sums of nl
+    int* offU = nullptr;      // device [N_r] prefix sums of (nu + 1)
+    size_t nL = 0, nU = 0;
+    std::vector<int> h_lo, h_hi, h_offL, h_offU;
+};
+
+struct Tables {               // all device pointers
+    double* D1 = nullptr;     // [N_r][9]   d/dr weights on the stencil s0[j]..s0[j]+8
+    double* L0 = nullptr;     // [N_r][9]   d2/dr2 + (1/r) d/dr
+    int* s0 = nullptr;        // [N_r]      first stencil node
+    double* Q = nullptr;      // [N_r][17]  (D1 + 1/r) G~ on columns q0[j]..q0[j]+16
+    int* q0 = nullptr;        // [N_r]
+    double* rinv = nullptr;   // [N_r]      1 / r_j
+    double* nm = nullptr;     // [M+1]      n = m k_theta0
+    double* kap = nullptr;    // [2K+1]     kappa = k alpha
+    cd* tw_t = nullptr;       // [N_theta]  exp(-2 pi i t / N_theta)
+    cd* tw_z = nullptr;       // [N_z]
+};
+
+}  // namespace nsc
+
+struct nsc_ctx {
+    nsc_params p{};
+    int N_r = 0, M = 0, K = 0, M1 = 0, NK = 0, MP = 0, Nt = 0, Nz = 0, nf = 3, JC = 0;
+    bool heated = false;
+    size_t F = 0;                         // complex elements per spectral field
+    int P = 0;                            // pairs (m, |k|): (M+1)(K+1)
+    cudaStream_t stream = nullptr;
+    std::vector<double> r;                // radial nodes (host copy)
+    nsc::Tables t;
+    nsc::cd* state[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // u_r, u_theta, u_z, T, p
+    nsc::cd* W[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};        // sub-step work / predictor state
+    nsc::cd* G = nullptr;                 // divergence / phi
+    nsc::cd* N0[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
+    nsc::cd* N1[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
+    nsc::cd* zbuf = nullptr;              // [3 nf][JC][N_z][MP]  z-transformed f, dz f, dr f
+    nsc::cd* tbuf = nullptr;              // [nf][JC][N_z][MP]    theta-transformed products
+    nsc::BandShape shH, shP;              // Helmholtz (9-wide rows) / Poisson (17-wide rows) envelopes
+    nsc::BandFactors facH[4];             // u_+, u_-, u_z, T
+    nsc::BandFactors facP;
+    bool facT_shared = false;             // T shares the u_z factors (Pr == 1)
+    double fac_dt = 0.0;                  // dt the Helmholtz factors were built for (0: none)
+    bool facP_ready = false;
+    bool have_state = false;
+    std::string err;
+    long long launches = 0;
+    long long dev_bytes = 0;
+    std::vector<void*> allocs;
+};
+
+namespace nsc {
+
+// plan.cu
+int build_plan(nsc_ctx* c);
+
+// nonlinear.cu : N(f[0..nf-1]) -> out[0..nf-1]   (steps N1-N6)
+int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out);
+
+// linear.cu
+int ensure_factors(nsc_ctx* c, double dt);
+// one implicit sub-step from c->state with explicit term w0*E0 + w1*E1 (E1 may be null);
+// result (u, T) -> dst[0..nf-1]; new pressure -> p_dst (may be null: discarded)
+int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w1, double dt,
+                   cd* const* dst, cd* p_dst);
+
+int fail(nsc_ctx* c, int code, const std::string& msg);
+int cuda_fail(nsc_ctx* c, cudaError_t e, const char* what);
+
+}  // namespace nsc
+
+#define NSC_CUDA(c, call)                                                  \
+    do {                                                                   \
+        cudaError_t e__ = (call);                                          \
+        if (e__ != cudaSuccess) return nsc::cuda_fail((c), e__, #call);    \
+    } while (0)

@@ -1,0 +1,202 @@
+"""Thin binding over the C-ABI library ``libnsc.so`` (include/nsc.h).
+
+Argument marshalling only: every step of the time step runs in the library's CUDA kernels.
+PyTorch supplies device memory and streams.  There is no fallback: if ``libnsc.so`` is missing
+(run ``python -m paper_1908_00587_b200.build``) or no CUDA device is present, calls raise.
+
+Names follow the header: ``nsc_create`` -> :class:`Context`, ``nsc_set_state``, ``nsc_nonlinear``,
+``nsc_substep``, ``nsc_step``, ``nsc_get_state``, ``nsc_destroy``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnsc.so")
+
+EXPORTS = (
+    "nsc_create", "nsc_create_ex", "nsc_destroy", "nsc_set_stream", "nsc_get_grid",
+    "nsc_set_state", "nsc_get_state", "nsc_set_state_host", "nsc_get_state_host",
+    "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_last_error", "nsc_device_bytes",
+    "nsc_launch_count",
+)
+
+NSC_OK, NSC_EINVAL, NSC_ENOMEM, NSC_ECUDA, NSC_ESTATE = 0, -1, -2, -3, -4
+
+
+class NscError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libnsc error {code}: {msg}")
+        self.code = code
+
+
+class nsc_params(C.Structure):
+    _fields_ = [
+        ("N_r", C.c_int), ("M_theta", C.c_int), ("K_z", C.c_int),
+        ("eta", C.c_double), ("alpha", C.c_double), ("k_theta0", C.c_int),
+        ("Re_i", C.c_double), ("Re_o", C.c_double), ("Ra", C.c_double), ("Pr", C.c_double),
+        ("radial_grid", C.c_int), ("n_theta_phys", C.c_int), ("n_z_phys", C.c_int),
+        ("c", C.c_double), ("device", C.c_int), ("radial_chunk", C.c_int),
+    ]
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """Loads libnsc.so (once) and declares the prototypes.  Raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_1908_00587_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, dbl, i32 = C.c_void_p, C.c_double, C.c_int
+    lib.nsc_create.argtypes = [C.POINTER(vp), i32, i32, i32, dbl, dbl, i32, dbl, dbl, dbl, dbl, i32]
+    lib.nsc_create_ex.argtypes = [C.POINTER(vp), C.POINTER(nsc_params)]
+    lib.nsc_destroy.argtypes = [vp]
+    lib.nsc_set_stream.argtypes = [vp, vp]
+    lib.nsc_get_grid.argtypes = [vp, C.POINTER(dbl)]
+    lib.nsc_set_state.argtypes = [vp] + [vp] * 5
+    lib.nsc_get_state.argtypes = [vp] + [vp] * 5
+    lib.nsc_set_state_host.argtypes = [vp] + [vp] * 5
+    lib.nsc_get_state_host.argtypes = [vp] + [vp] * 5
+    lib.nsc_nonlinear.argtypes = [vp] + [vp] * 4
+    lib.nsc_substep.argtypes = [vp] + [vp] * 4 + [dbl]
+    lib.nsc_step.argtypes = [vp, dbl]
+    lib.nsc_last_error.argtypes = [vp]
+    lib.nsc_last_error.restype = C.c_char_p
+    lib.nsc_device_bytes.argtypes = [vp]
+    lib.nsc_device_bytes.restype = C.c_longlong
+    lib.nsc_launch_count.argtypes = [vp]
+    lib.nsc_launch_count.restype = C.c_longlong
+    for name in EXPORTS:
+        if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count"):
+            getattr(lib, name).restype = i32
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    """Device (torch.Tensor) or host (numpy.ndarray) complex128 buffer -> void*; None -> NULL."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.complex128 or not t.flags["C_CONTIGUOUS"]:
+            raise ValueError("host buffers must be C-contiguous complex128")
+        return C.c_void_p(t.ctypes.data)
+    import torch
+    if t.dtype != torch.complex128 or not t.is_contiguous():
+        raise ValueError("device buffers must be contiguous complex128")
+    return C.c_void_p(t.data_ptr())
+
+
+class Context:
+    """One Taylor-Couette configuration on one GPU (``nsc_create`` ... ``nsc_destroy``)."""
+
+    def __init__(self, N_r, M, K, eta, alpha, k_theta0, Re_i, Re_o, Ra=0.0, Pr=1.0, grid=1,
+                 n_theta=0, n_z=0, c=0.0, device=-1, radial_chunk=0):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        p = nsc_params(N_r, M, K, eta, alpha, k_theta0, Re_i, Re_o, Ra, Pr, grid, n_theta, n_z, c,
+                       device, radial_chunk)
+        rc = self._lib.nsc_create_ex(C.byref(self._h), C.byref(p))
+        if rc != NSC_OK:
+            msg = self._lib.nsc_last_error(None).decode()
+            self._h = None
+            raise NscError(rc, msg)
+        self.N_r, self.M, self.K = N_r, M, K
+        self.heated = Ra != 0.0
+        self.nf = 4 if self.heated else 3
+        self.shape = (N_r, M + 1, 2 * K + 1)
+
+    @classmethod
+    def from_config(cls, cfg: dict, **over):
+        keys = ("N_r", "M", "K", "eta", "alpha", "k_theta0", "Re_i", "Re_o", "Ra", "Pr", "grid")
+        kw = {k: cfg[k] for k in keys}
+        kw.update(over)
+        return cls(**kw)
+
+    # ------------------------------------------------------------------ plumbing
+    def _check(self, rc):
+        if rc != NSC_OK:
+            raise NscError(rc, self._lib.nsc_last_error(self._h).decode())
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.nsc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def set_stream(self, stream=None):
+        """Enqueue all later work on ``stream`` (a torch.cuda.Stream; None: torch's current)."""
+        import torch
+        s = stream if stream is not None else torch.cuda.current_stream()
+        self._check(self._lib.nsc_set_stream(self._h, C.c_void_p(s.cuda_stream)))
+
+    def grid(self) -> np.ndarray:
+        r = np.empty(self.N_r, np.float64)
+        self._check(self._lib.nsc_get_grid(self._h, r.ctypes.data_as(C.POINTER(C.c_double))))
+        return r
+
+    def empty(self, n=1):
+        import torch
+        out = [torch.empty(self.shape, dtype=torch.complex128, device="cuda") for _ in range(n)]
+        return out[0] if n == 1 else out
+
+    # ------------------------------------------------------------------ the ABI calls
+    def set_state(self, ur, uth, uz, T=None, p=None):
+        host = isinstance(ur, np.ndarray)
+        fn = self._lib.nsc_set_state_host if host else self._lib.nsc_set_state
+        self._check(fn(self._h, _ptr(ur), _ptr(uth), _ptr(uz), _ptr(T), _ptr(p)))
+
+    def get_state(self, ur=None, uth=None, uz=None, T=None, p=None):
+        host = any(isinstance(a, np.ndarray) for a in (ur, uth, uz, T, p))
+        fn = self._lib.nsc_get_state_host if host else self._lib.nsc_get_state
+        self._check(fn(self._h, _ptr(ur), _ptr(uth), _ptr(uz), _ptr(T), _ptr(p)))
+
+    def nonlinear(self, Nr, Nth, Nz, NT=None):
+        self._check(self._lib.nsc_nonlinear(self._h, _ptr(Nr), _ptr(Nth), _ptr(Nz), _ptr(NT)))
+
+    def substep(self, Er, Eth, Ez, ET, dt):
+        self._check(self._lib.nsc_substep(self._h, _ptr(Er), _ptr(Eth), _ptr(Ez), _ptr(ET), float(dt)))
+
+    def step(self, dt):
+        self._check(self._lib.nsc_step(self._h, float(dt)))
+
+    def device_bytes(self) -> int:
+        return int(self._lib.nsc_device_bytes(self._h))
+
+    def launch_count(self) -> int:
+        return int(self._lib.nsc_launch_count(self._h))
+
+    # ------------------------------------------------------------------ conveniences (copies only)
+    def state_to_host(self):
+        """Current state as numpy arrays [u_r, u_theta, u_z, T or None, p]."""
+        out = [np.empty(self.shape, np.complex128) for _ in range(5)]
+        if not self.heated:
+            out[3] = None
+        self.get_state(*out)
+        return out
+
+    def nonlinear_to_host(self):
+        import torch
+        bufs = self.empty(self.nf)
+        self.nonlinear(*bufs)
+        torch.cuda.synchronize()
+        return [b.cpu().numpy() for b in bufs]

@@ -1,0 +1,179 @@
+"""GPU parity (-m gpu): the CUDA path, called through the C ABI, against the oracle on the same
+seeded inputs.  Tolerances are BASELINE.json north_star's: relative L2 (norm R14, all fields
+concatenated, base flow included) <= 1e-11 per nonlinear evaluation, <= 1e-9 after 20 steps."""
+import numpy as np
+import pytest
+
+from helpers import oracle_of, nf_of
+from oracle.nsc_oracle import rel_l2
+from paper_1908_00587_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_N = 1e-11
+TOL_STEP = 1e-9
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1908_00587_b200 import build
+    build.build()
+    return torch
+
+
+def _ctx(cfg, **over):
+    from paper_1908_00587_b200 import nsc
+    return nsc.Context.from_config(cfg, **over)
+
+
+def _dev(torch, arrs):
+    return [None if a is None else torch.from_numpy(a).cuda() for a in arrs]
+
+
+def _random_fields(cfg, seed, n):
+    rng = np.random.default_rng(seed)
+    shp = (cfg["N_r"], cfg["M"] + 1, 2 * cfg["K"] + 1)
+    out = []
+    for _ in range(n):
+        f = rng.standard_normal(shp) + 1j * rng.standard_normal(shp)
+        out.append(np.ascontiguousarray(f))
+    return out
+
+
+# (config index, N_r, M, K, oracle DFT backend): spans every transform length 12 .. 1536, several
+# line tiles per CTA with ragged tails (N_r * (M+1) and N_r * N_z not multiples of the tile)
+NL_CASES = [
+    (0, 32, 8, 8, "naive"),       # cfg 1 as is
+    (2, 11, 4, 16, "naive"),      # heated; lengths 12 / 48
+    (1, 13, 32, 32, "naive"),     # lengths 96 / 96
+    (2, 10, 64, 8, "naive"),      # heated; 192 / 24
+    (3, 9, 128, 4, "fft"),        # 384 / 12
+    (3, 12, 256, 8, "fft"),       # 768 / 24  (cfg 4's theta length)
+    (1, 10, 8, 256, "fft"),       # 24 / 768  (cfg 4's z length)
+    (4, 9, 512, 4, "fft"),        # heated; 1536 / 12 (cfg 5's theta length)
+    (4, 9, 4, 512, "fft"),        # heated; 12 / 1536
+]
+
+
+@pytest.mark.parametrize("ci,N_r,M,K,dft", NL_CASES)
+def test_nonlinear_matches_oracle(torch_cuda, ci, N_r, M, K, dft):
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    o = oracle_of(cfg, dft=dft)
+    with _ctx(cfg) as ctx:
+        np.testing.assert_array_equal(ctx.grid(), o.r)        # same nodes, bit for bit
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        got = ctx.nonlinear_to_host()
+    ref = o.nonlinear(*st[:nf_of(cfg)])
+    assert rel_l2(got, ref) <= TOL_N
+
+
+def test_nonlinear_broadband_random_fields_and_chunking(torch_cuda):
+    """Full-band random (non-smooth, non-Hermitian m = 0 row) fields; radial chunking of the
+    transform pipeline must not change a bit."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(2, N_r=21, M=16, K=8)
+    o = oracle_of(cfg)
+    fs = _random_fields(cfg, 5, 4)
+    ref = o.nonlinear(*fs)
+    res = []
+    for chunk in (0, 4, 1):
+        with _ctx(cfg, radial_chunk=chunk) as ctx:
+            ctx.set_state(*_dev(torch, fs), None)
+            res.append(ctx.nonlinear_to_host())
+    assert rel_l2(res[0], ref) <= TOL_N
+    for other in res[1:]:
+        for a, b in zip(res[0], other):
+            np.testing.assert_array_equal(a, b)
+
+
+def test_nonlinear_padded_grid_variant(torch_cuda):
+    """cfg 1 on the 24 x 48 grid BASELINE.json quotes (reading R4): equal to the oracle on that
+    grid, and equal to the 24 x 24 result away from |k| = K."""
+    torch = torch_cuda
+    cfg = synth.config(0)
+    o = oracle_of(cfg, n_z=48)
+    with _ctx(cfg, n_z=48) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        got = ctx.nonlinear_to_host()
+    assert rel_l2(got, o.nonlinear(*st[:3])) <= TOL_N
+
+
+SUB_CASES = [(0, 32, 8, 8), (2, 24, 4, 8), (1, 64, 8, 4), (3, 40, 4, 4), (2, 9, 4, 4)]
+
+
+@pytest.mark.parametrize("ci,N_r,M,K", SUB_CASES)
+def test_substep_matches_oracle(torch_cuda, ci, N_r, M, K):
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    nf = nf_of(cfg)
+    o = oracle_of(cfg)
+    with _ctx(cfg) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        rng = np.random.default_rng(3)
+        st[4] = 10.0 * (rng.standard_normal(st[0].shape) + 1j * rng.standard_normal(st[0].shape))
+        U = max(abs(cfg["Re_i"]), abs(cfg["Re_o"]))
+        E = [U * U * 0.1 * f for f in _random_fields(cfg, 8, nf)]
+        ctx.set_state(*_dev(torch, st))
+        Ed = _dev(torch, E) + [None] * (4 - nf)
+        ctx.substep(*Ed, cfg["dt"])
+        got = ctx.state_to_host()
+    ref = o.substep(st, E, cfg["dt"])
+    assert rel_l2(got[:nf], ref[:nf]) <= 1e-11
+    assert rel_l2([got[4]], [ref[4]]) <= 1e-7       # pressure: parity unpinned (phi / dt amplifies round-off)
+
+
+@pytest.mark.parametrize("ci,N_r,M,K,nsteps", [(0, 32, 8, 8, 20), (2, 32, 8, 8, 20), (1, 64, 32, 32, 5)])
+def test_steps_match_oracle(torch_cuda, ci, N_r, M, K, nsteps):
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    nf = nf_of(cfg)
+    o = oracle_of(cfg, dft="fft")
+    with _ctx(cfg) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        for _ in range(nsteps):
+            ctx.step(cfg["dt"])
+        got = ctx.state_to_host()
+    ref = st
+    for _ in range(nsteps):
+        ref = o.step(ref, cfg["dt"])
+    assert rel_l2(got[:nf], ref[:nf]) <= TOL_STEP
+
+
+def test_couette_flow_is_a_fixed_point_on_the_gpu(torch_cuda):
+    torch = torch_cuda
+    cfg = synth.scaled_config(0, N_r=32, M=4, K=4)
+    o = oracle_of(cfg)
+    base = o.base_state_discrete()
+    with _ctx(cfg) as ctx:
+        ctx.set_state(*_dev(torch, base))
+        for _ in range(3):
+            ctx.step(1e-2)
+        got = ctx.state_to_host()
+    assert rel_l2(got[:3], base[:3]) <= 1e-13
+
+
+def test_host_buffer_entry_points_and_errors(torch_cuda):
+    from paper_1908_00587_b200 import nsc
+    cfg = synth.scaled_config(0, N_r=16, M=4, K=4)
+    with _ctx(cfg) as ctx:
+        with pytest.raises(nsc.NscError) as ei:
+            ctx.step(1e-3)
+        assert ei.value.code == nsc.NSC_ESTATE
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*st)                         # numpy arrays -> nsc_set_state_host
+        back = ctx.state_to_host()
+        for a, b in zip(st, back):
+            if a is not None:
+                np.testing.assert_array_equal(a, b)
+        with pytest.raises(nsc.NscError) as ei:
+            ctx.step(-1.0)
+        assert ei.value.code == nsc.NSC_EINVAL
+        assert ctx.launch_count() == 0
+        ctx.step(1e-3)
+        assert ctx.launch_count() > 0
