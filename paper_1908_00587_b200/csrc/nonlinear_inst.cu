@@ -13,8 +13,9 @@ namespace nsc {
 #define NSC_CAT(a, b) NSC_CAT2(a, b)
 constexpr int LEN = NSC_FFT_N;
 
-template <class Kern> static int prep(Kern k, size_t smem) {
-    static bool done = false;          // per kernel (template instance of this function)
+// raises the dynamic shared-memory limit of kernel k once (ID = one flag per kernel)
+template <int ID, class Kern> static int prep(Kern k, size_t smem) {
+    static bool done = false;
     if (!done) {
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return (int)e;
@@ -25,7 +26,7 @@ template <class Kern> static int prep(Kern k, size_t smem) {
 
 int NSC_CAT(launch_zinv_, NSC_FFT_N)(const NlArgs& a, cudaStream_t st) {
     using C = ZCfg<LEN>;
-    if (int e = prep(k_zinv<LEN>, C::SMEM)) return e;
+    if (int e = prep<0>(k_zinv<LEN>, C::SMEM)) return e;
     const int nlines = a.nj * a.M1;
     dim3 grid((nlines + C::LPC - 1) / C::LPC, a.nf);
     k_zinv<LEN><<<grid, C::THREADS, C::SMEM, st>>>(a);
@@ -34,7 +35,7 @@ int NSC_CAT(launch_zinv_, NSC_FFT_N)(const NlArgs& a, cudaStream_t st) {
 
 int NSC_CAT(launch_zfwd_, NSC_FFT_N)(const NlArgs& a, cudaStream_t st) {
     using C = ZCfg<LEN>;
-    if (int e = prep(k_zfwd<LEN>, C::SMEM)) return e;
+    if (int e = prep<1>(k_zfwd<LEN>, C::SMEM)) return e;
     const int nlines = a.nj * a.M1;
     dim3 grid((nlines + C::LPC - 1) / C::LPC, a.nf);
     k_zfwd<LEN><<<grid, C::THREADS, C::SMEM, st>>>(a);
@@ -46,10 +47,10 @@ int NSC_CAT(launch_theta_, NSC_FFT_N)(const NlArgs& a, cudaStream_t st) {
     const int nlines = a.nj * a.Nz;
     dim3 grid((nlines + C::LPC - 1) / C::LPC);
     if (a.nf == 3) {
-        if (int e = prep(k_theta<LEN, 3>, C::SMEM)) return e;
+        if (int e = prep<2>(k_theta<LEN, 3>, C::SMEM)) return e;
         k_theta<LEN, 3><<<grid, C::THREADS, C::SMEM, st>>>(a);
     } else {
-        if (int e = prep(k_theta<LEN, 4>, C::SMEM)) return e;
+        if (int e = prep<3>(k_theta<LEN, 4>, C::SMEM)) return e;
         k_theta<LEN, 4><<<grid, C::THREADS, C::SMEM, st>>>(a);
     }
     return (int)cudaGetLastError();
