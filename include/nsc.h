@@ -122,6 +122,28 @@ long long nsc_device_bytes(const nsc_ctx* ctx);
 /* Number of kernel launches this context has enqueued so far (for bench.py's gpu_launches). */
 long long nsc_launch_count(const nsc_ctx* ctx);
 
+/* Per-kernel device timing (for bench.py's roofline figures).  With profiling on, every kernel
+ * launch is bracketed by CUDA events on the context's stream.  nsc_profile_read synchronises the
+ * stream, ADDS the elapsed milliseconds and launch counts since the last read to h_ms[id] /
+ * h_count[id] (host arrays of NSC_NKERN entries; the caller zeroes them) and forgets the events.
+ * Kernel ids are the NSC_K_* constants; nsc_kernel_name gives the kernel's name. */
+enum {
+    NSC_K_ZINV = 0,      /* N1 + N2: z-derivative, radial derivative, padded inverse z-FFT          */
+    NSC_K_THETA = 1,     /* N1 + N3 + N4 + N5: fused theta transforms and physical-space products   */
+    NSC_K_ZFWD = 2,      /* N6: forward z-FFT, truncation, scaling, buoyancy                         */
+    NSC_K_RHS = 3,       /* L1                                                                       */
+    NSC_K_HELMHOLTZ = 4, /* L2: banded solves for u_+, u_-, u_z, T                                  */
+    NSC_K_RECOMBINE = 5, /* L3a                                                                      */
+    NSC_K_DIV = 6,       /* L3b                                                                      */
+    NSC_K_POISSON = 7,   /* L4                                                                       */
+    NSC_K_CORRECT = 8,   /* L5                                                                       */
+    NSC_K_FACTOR = 9,    /* set-up: banded LU of the per-mode matrices (once per dt)                 */
+    NSC_NKERN = 10
+};
+int nsc_set_profiling(nsc_ctx* ctx, int on);
+int nsc_profile_read(nsc_ctx* ctx, double* h_ms, long long* h_count);
+const char* nsc_kernel_name(int id);
+
 #ifdef __cplusplus
 }
 #endif

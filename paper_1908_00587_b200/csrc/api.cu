@@ -40,6 +40,34 @@ static int dev_alloc(nsc_ctx* c, cd** dst, size_t elems, bool zero) {
     return NSC_OK;
 }
 
+static cudaEvent_t get_event(nsc_ctx* c) {
+    if (!c->ev_pool.empty()) {
+        cudaEvent_t e = c->ev_pool.back();
+        c->ev_pool.pop_back();
+        return e;
+    }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+
+void prof_begin(nsc_ctx* c, int kernel_id) {
+    c->launches += 1;
+    if (!c->profiling) return;
+    nsc_ctx::ProfRec r{kernel_id, get_event(c), get_event(c)};
+    cudaEventRecord(r.a, c->stream);
+    c->prof.push_back(r);
+}
+
+void prof_end(nsc_ctx* c) {
+    if (!c->profiling) return;
+    cudaEventRecord(c->prof.back().b, c->stream);
+}
+
+static const char* kKernelNames[NSC_NKERN] = {"k_zinv", "k_theta", "k_zfwd", "k_rhs", "k_band_solve<helmholtz>",
+                                              "k_recombine", "k_div", "k_band_solve<poisson>", "k_correct",
+                                              "k_factor"};
+
 static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
 
 }  // namespace nsc
@@ -147,6 +175,11 @@ int nsc_destroy(nsc_ctx* c) {
     if (!c) return NSC_OK;
     cudaDeviceSynchronize();
     for (void* p : c->allocs) cudaFree(p);
+    for (auto& r : c->prof) {
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     cudaGetLastError();
     delete c;
     return NSC_OK;
@@ -246,6 +279,29 @@ int nsc_step(nsc_ctx* c, double dt) {
     if ((rc = launch_nonlinear(c, c->W, c->N1))) return rc;
     return launch_substep(c, c->N1, c->p.c, c->N0, 1.0 - c->p.c, dt, c->state, c->state[4]);
 }
+
+int nsc_set_profiling(nsc_ctx* c, int on) {
+    if (!c) return NSC_EINVAL;
+    c->profiling = on != 0;
+    return NSC_OK;
+}
+
+int nsc_profile_read(nsc_ctx* c, double* h_ms, long long* h_count) {
+    if (!c || !h_ms || !h_count) return NSC_EINVAL;
+    NSC_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (auto& r : c->prof) {
+        float ms = 0.f;
+        NSC_CUDA(c, cudaEventElapsedTime(&ms, r.a, r.b));
+        h_ms[r.id] += ms;
+        h_count[r.id] += 1;
+        c->ev_pool.push_back(r.a);
+        c->ev_pool.push_back(r.b);
+    }
+    c->prof.clear();
+    return NSC_OK;
+}
+
+const char* nsc_kernel_name(int id) { return (id >= 0 && id < NSC_NKERN) ? kKernelNames[id] : ""; }
 
 const char* nsc_last_error(const nsc_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
 

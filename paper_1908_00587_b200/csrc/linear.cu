@@ -376,8 +376,9 @@ static int run_factor(nsc_ctx* c, BandFactors& f, const BandShape& s, int kind, 
     a.kind = kind;
     a.coef = coef;
     a.shift = shift;
+    prof_begin(c, NSC_K_FACTOR);
     k_factor<<<(c->P + 63) / 64, 64, 0, c->stream>>>(a);
-    c->launches += 1;
+    prof_end(c);
     NSC_CUDA(c, cudaGetLastError());
     return NSC_OK;
 }
@@ -422,11 +423,12 @@ static int run_solve(nsc_ctx* c, const BandFactors& f, const BandShape& s, cd* x
     a.P = c->P;
     const int threads = 128;
     const int blocks = (c->P + threads - 1) / threads;
+    prof_begin(c, poisson ? NSC_K_POISSON : NSC_K_HELMHOLTZ);
     if (poisson)
         k_band_solve<8, 12><<<blocks, threads, 0, c->stream>>>(a);
     else
         k_band_solve<4, 8><<<blocks, threads, 0, c->stream>>>(a);
-    c->launches += 1;
+    prof_end(c);
     NSC_CUDA(c, cudaGetLastError());
     return NSC_OK;
 }
@@ -466,21 +468,26 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
     a.Re_o = c->p.Re_o;
     const int plane = c->M1 * c->NK;
     dim3 gridp((plane + 127) / 128, c->N_r);
+    prof_begin(c, NSC_K_RHS);
     k_rhs<<<gridp, 128, 0, c->stream>>>(a);
-    c->launches += 1;
+    prof_end(c);
     NSC_CUDA(c, cudaGetLastError());
     if ((rc = run_solve(c, c->facH[0], c->shH, c->W[0], false))) return rc;
     if ((rc = run_solve(c, c->facH[1], c->shH, c->W[1], false))) return rc;
     if ((rc = run_solve(c, c->facH[2], c->shH, c->W[2], false))) return rc;
     if (c->heated)
         if ((rc = run_solve(c, c->facT_shared ? c->facH[2] : c->facH[3], c->shH, c->W[3], false))) return rc;
+    prof_begin(c, NSC_K_RECOMBINE);
     k_recombine<<<(unsigned)((c->F + 255) / 256), 256, 0, c->stream>>>(a, c->F);
+    prof_end(c);
+    prof_begin(c, NSC_K_DIV);
     k_div<<<gridp, 128, 0, c->stream>>>(a);
-    c->launches += 2;
+    prof_end(c);
     NSC_CUDA(c, cudaGetLastError());
     if ((rc = run_solve(c, c->facP, c->shP, c->G, true))) return rc;
+    prof_begin(c, NSC_K_CORRECT);
     k_correct<<<gridp, 128, 0, c->stream>>>(a);
-    c->launches += 1;
+    prof_end(c);
     NSC_CUDA(c, cudaGetLastError());
     return NSC_OK;
 }

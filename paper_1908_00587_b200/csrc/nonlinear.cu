@@ -53,12 +53,17 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
         a.j0 = j0;
         a.nj = (c->N_r - j0 < c->JC) ? c->N_r - j0 : c->JC;
         a.tw = c->t.tw_z;
+        prof_begin(c, NSC_K_ZINV);
         if (int e = lz->zinv(a, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zinv launch");
+        prof_end(c);
         a.tw = c->t.tw_t;
+        prof_begin(c, NSC_K_THETA);
         if (int e = lt->theta(a, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_theta launch");
+        prof_end(c);
         a.tw = c->t.tw_z;
+        prof_begin(c, NSC_K_ZFWD);
         if (int e = lz->zfwd(a, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zfwd launch");
-        c->launches += 3;
+        prof_end(c);
     }
     return NSC_OK;
 }

@@ -74,6 +74,11 @@ struct nsc_ctx {
     long long launches = 0;
     long long dev_bytes = 0;
     std::vector<void*> allocs;
+    // optional per-kernel event timing (nsc_set_profiling)
+    struct ProfRec { int id; cudaEvent_t a, b; };
+    bool profiling = false;
+    std::vector<ProfRec> prof;
+    std::vector<cudaEvent_t> ev_pool;
 };
 
 namespace nsc {
@@ -90,6 +95,11 @@ int ensure_factors(nsc_ctx* c, double dt);
 // result (u, T) -> dst[0..nf-1]; new pressure -> p_dst (may be null: discarded)
 int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w1, double dt,
                    cd* const* dst, cd* p_dst);
+
+// event brackets around a kernel launch (no-ops unless profiling is on); every launch site uses
+// them, and they also count the launch.
+void prof_begin(nsc_ctx* c, int kernel_id);
+void prof_end(nsc_ctx* c);
 
 int fail(nsc_ctx* c, int code, const std::string& msg);
 int cuda_fail(nsc_ctx* c, cudaError_t e, const char* what);

@@ -21,8 +21,9 @@ EXPORTS = (
     "nsc_create", "nsc_create_ex", "nsc_destroy", "nsc_set_stream", "nsc_get_grid",
     "nsc_set_state", "nsc_get_state", "nsc_set_state_host", "nsc_get_state_host",
     "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_last_error", "nsc_device_bytes",
-    "nsc_launch_count",
+    "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name",
 )
+NSC_NKERN = 10
 
 NSC_OK, NSC_EINVAL, NSC_ENOMEM, NSC_ECUDA, NSC_ESTATE = 0, -1, -2, -3, -4
 
@@ -74,8 +75,12 @@ def load_library() -> C.CDLL:
     lib.nsc_device_bytes.restype = C.c_longlong
     lib.nsc_launch_count.argtypes = [vp]
     lib.nsc_launch_count.restype = C.c_longlong
+    lib.nsc_set_profiling.argtypes = [vp, i32]
+    lib.nsc_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(C.c_longlong)]
+    lib.nsc_kernel_name.argtypes = [i32]
+    lib.nsc_kernel_name.restype = C.c_char_p
     for name in EXPORTS:
-        if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count"):
+        if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count", "nsc_kernel_name"):
             getattr(lib, name).restype = i32
     _lib = lib
     return lib
@@ -184,6 +189,16 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self._lib.nsc_launch_count(self._h))
+
+    def set_profiling(self, on: bool):
+        self._check(self._lib.nsc_set_profiling(self._h, int(bool(on))))
+
+    def profile_read(self) -> dict:
+        """{kernel name: (milliseconds, launches)} accumulated since the last read."""
+        ms = (C.c_double * NSC_NKERN)()
+        cnt = (C.c_longlong * NSC_NKERN)()
+        self._check(self._lib.nsc_profile_read(self._h, ms, cnt))
+        return {self._lib.nsc_kernel_name(i).decode(): (ms[i], cnt[i]) for i in range(NSC_NKERN)}
 
     # ------------------------------------------------------------------ conveniences (copies only)
     def state_to_host(self):
