@@ -138,7 +138,8 @@ enum {
     NSC_K_POISSON = 7,   /* L4                                                                       */
     NSC_K_CORRECT = 8,   /* L5                                                                       */
     NSC_K_FACTOR = 9,    /* set-up: banded LU of the per-mode matrices (once per dt)                 */
-    NSC_NKERN = 10
+    NSC_K_DR = 10,       /* N1: radial derivative of the spectral fields (length-768 pipeline only)  */
+    NSC_NKERN = 11
 };
 int nsc_set_profiling(nsc_ctx* ctx, int on);
 int nsc_profile_read(nsc_ctx* ctx, double* h_ms, long long* h_count);

@@ -2,6 +2,7 @@
 // one predictor-corrector step (O7) from the kernels of nonlinear.cu
 // and linear.cu.  No arithmetic of the method happens on the host after nsc_create.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include "nsc_internal.h"
@@ -66,7 +67,7 @@ void prof_end(nsc_ctx* c) {
 
 static const char* kKernelNames[NSC_NKERN] = {"k_zinv", "k_theta", "k_zfwd", "k_rhs", "k_band_solve<helmholtz>",
                                               "k_recombine", "k_div", "k_band_solve<poisson>", "k_correct",
-                                              "k_factor"};
+                                              "k_factor", "k_dr"};
 
 static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
 
@@ -128,7 +129,18 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
     if (jc > c->N_r) jc = c->N_r;
     c->JC = jc;
 
+    // length-768 transform pipeline (nonlinear_v2.cuh); NSC_NL_VARIANT (experiments): bit 0 = z kernels,
+    // bits 1-2 = theta kernel (1 shared-memory scratch, 2 TMEM scratch); default 1 | 2 << 1
+    {
+        int variant = 1 | (2 << 1);
+        if (const char* ev = getenv("NSC_NL_VARIANT")) variant = atoi(ev);
+        c->z768 = (variant & 1) && c->Nz == 768 && c->K <= 256 && c->MP % 4 == 0;
+        c->t768 = (c->Nt == 768 && c->M <= 256 && c->nf == 3) ? ((variant >> 1) & 3) : 0;
+        if (c->t768 > 2) c->t768 = 2;
+    }
     int rc = build_plan(c);
+    if (!rc && c->z768)
+        for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->DR[i], c->F, false);
     if (!rc) {
         for (int i = 0; i < 5 && !rc; ++i)
             if (i != 3 || c->heated) rc = dev_alloc(c, &c->state[i], c->F, true);

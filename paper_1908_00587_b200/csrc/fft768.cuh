@@ -1,0 +1,190 @@
+// fft768.cuh -- two-pass fp64 FFT of length 768 = 24 x 32 for one warp per line.
+//
+// The headline workload (BASELINE.json configs[3]: 768 x 768 physical grid per radial node) spends
+// its time in length-768 transforms.  With 24 complex values per thread the
+// generic three-pass plan of fft.cuh exchanges every line twice through shared memory and is bound
+// by the shared-memory crossbar (128 B/clk/SM), not by the DFMA pipe.  Here a line crosses shared
+// memory ONCE:
+//
+//   "S" (spectral-side) layout : 32 lanes x 24 values, lane tau holds line index tau + 32 t, t < 24
+//   "P" (physical-side) layout : 24 lanes x 32 values, lane a   holds line index a + 24 p(e), e < 32,
+//                                p(e) = (e >> 3) + 4 (e & 7)   (register order left by the radix-32
+//                                butterfly; a static permutation, never materialised)
+//
+//   s2p :  S -> P     n = 32 n1 + tau,  k = a + 24 k2
+//          pass A  lane tau: DFT-24 over n1 (Good-Thomas 3 x 8, no inner twiddles), times W_768^(tau k1)
+//          exchange through a [24][33] complex matrix (row = k1 = a, column = tau; stride 33 keeps
+//          both the column-wise 16-byte stores and the row-wise 16-byte loads conflict free)
+//          pass B  lane a < 24: DFT-32 over tau (4 x 8 with W_32 constants)
+//   p2s :  P -> S     n = a + 24 n2,  k = 32 k1 + tau      (the mirror image)
+//
+// Lanes 24..31 idle through the radix-32 halves (they recompute lane 23's butterfly and store
+// nothing), which costs DFMA issue slots only while the crossbar, the actual bound, moves no byte
+// for them.  X[k] = sum_n x[n] exp(DIR 2 pi i n k / 768), unnormalised.
+#pragma once
+#include "fft.cuh"
+
+namespace nsc {
+namespace f768 {
+
+constexpr int N = 768;
+constexpr int NA = 24;            // radix of the pass on the S side
+constexpr int NB = 32;            // radix of the pass on the P side
+constexpr int XS = 33;            // row stride (complex) of the exchange matrix and the twiddle table
+constexpr int XBUF = NA * XS;     // complex elements of one exchange matrix (12 672 bytes)
+
+// physical line index of register e of lane a in the P layout
+NSC_HD int p_of(int e) { return (e >> 3) + 4 * (e & 7); }
+NSC_HD int p_idx(int e, int a) { return a + NA * p_of(e); }
+// line index of register t of lane tau in the S layout
+NSC_HD int s_idx(int t, int tau) { return tau + NB * t; }
+
+// cos / sin of 2 pi e / 32, correctly rounded
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+constexpr double cos32(int e) {
+    e &= 31;
+    if (e > 16) e = 32 - e;          // cos is even
+    bool neg = false;
+    if (e > 8) {
+        e = 16 - e;                  // cos(pi - x) = -cos(x)
+        neg = true;
+    }
+    double c = e == 0   ? 1.0
+               : e == 1 ? 0.98078528040323044912618223613424
+               : e == 2 ? 0.92387953251128675612818318939679
+               : e == 3 ? 0.83146961230254523707878837761791
+               : e == 4 ? 0.70710678118654752440084436210485
+               : e == 5 ? 0.55557023301960222474283081394853
+               : e == 6 ? 0.38268343236508977172845998403040
+               : e == 7 ? 0.19509032201612826784828486847702
+                        : 0.0;
+    return neg ? -c : c;
+}
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+constexpr double sin32(int e) { return cos32(e - 8); }
+
+// a * exp(DIR 2 pi i E / 32)
+template <int DIR, int E> NSC_HD cd mul_w32(cd a) {
+    constexpr int e = ((DIR > 0 ? E : -E) % 32 + 32) % 32;
+    if constexpr (e == 0) {
+        return a;
+    } else if constexpr (e == 8) {
+        return mul_i(a);
+    } else if constexpr (e == 16) {
+        return mk(-a.x, -a.y);
+    } else if constexpr (e == 24) {
+        return mul_mi(a);
+    } else if constexpr (e % 8 == 4) {
+        constexpr double h = 0.70710678118654752440084436210485;
+        // (+-1 +- i) / sqrt2
+        if constexpr (e == 4) return mk(h * (a.x - a.y), h * (a.x + a.y));
+        if constexpr (e == 12) return mk(-h * (a.x + a.y), h * (a.x - a.y));
+        if constexpr (e == 20) return mk(h * (a.y - a.x), -h * (a.x + a.y));
+        return mk(h * (a.x + a.y), h * (a.y - a.x));     // e == 28
+    } else {
+        constexpr double c = cos32(e), s = sin32(e);
+        return mk(a.x * c - a.y * s, a.x * s + a.y * c);
+    }
+}
+
+template <int DIR, int NBI, int KA> struct TwRow32 {
+    static NSC_HD void run(cd* x) {
+        if constexpr (NBI < 8) {
+            x[NBI + 8 * KA] = mul_w32<DIR, NBI * KA>(x[NBI + 8 * KA]);
+            TwRow32<DIR, NBI + 1, KA>::run(x);
+        }
+    }
+};
+
+// DFT-32, natural register order in (x[n]), permuted order out: x[8 ka + kb] = X[ka + 4 kb]
+template <int DIR> NSC_HD void dft32_nat_in(cd* x) {
+#pragma unroll
+    for (int nb = 0; nb < 8; ++nb) dft4<DIR>(x[nb], x[nb + 8], x[nb + 16], x[nb + 24]);
+    TwRow32<DIR, 1, 1>::run(x);
+    TwRow32<DIR, 1, 2>::run(x);
+    TwRow32<DIR, 1, 3>::run(x);
+#pragma unroll
+    for (int ka = 0; ka < 4; ++ka) dft8<DIR>(x + 8 * ka);
+}
+
+// DFT-32, permuted register order in (x[8 na + nb] = sample na + 4 nb), natural order out (x[k] = X[k])
+template <int DIR> NSC_HD void dft32_perm_in(cd* x) {
+#pragma unroll
+    for (int na = 0; na < 4; ++na) dft8<DIR>(x + 8 * na);
+    // x[8 na + kb] *= W_32^(na kb): the same table as above with the roles (ka, nb) -> (na, kb)
+    TwRow32<DIR, 1, 1>::run(x);
+    TwRow32<DIR, 1, 2>::run(x);
+    TwRow32<DIR, 1, 3>::run(x);
+#pragma unroll
+    for (int kb = 0; kb < 8; ++kb) dft4<DIR>(x[kb], x[kb + 8], x[kb + 16], x[kb + 24]);
+}
+
+// ---------------------------------------------------------------- phases of the two transforms
+// tw[k1 * XS + n2] = exp(-2 pi i k1 n2 / 768), k1 < 24, n2 < 32
+
+// s2p, lane tau < 32: x[0..23] (S layout) -> DFT-24, twiddle, store column tau of the matrix
+template <int DIR> NSC_HD void s2p_front(cd* x, cd* buf, const cd* tw, int tau) {
+    Dft<24, DIR>::run(x);
+#pragma unroll
+    for (int k1 = 1; k1 < NA; ++k1) {
+        cd w = tw[k1 * XS + tau];
+        if (DIR > 0) w = conj(w);
+        x[k1] = x[k1] * w;
+    }
+#pragma unroll
+    for (int k1 = 0; k1 < NA; ++k1) buf[k1 * XS + tau] = x[k1];
+}
+// s2p, lane a < 24 (callers pass a = min(tau, 23)): load row a, DFT-32 -> x[0..31] (P layout)
+template <int DIR> NSC_HD void s2p_back(cd* x, const cd* buf, int a) {
+#pragma unroll
+    for (int n2 = 0; n2 < NB; ++n2) x[n2] = buf[a * XS + n2];
+    dft32_nat_in<DIR>(x);
+}
+
+// p2s, lane a < 24: x[0..31] (P layout) -> DFT-32, twiddle, store row a  (store iff `active`)
+template <int DIR> NSC_HD void p2s_front(cd* x, cd* buf, const cd* tw, int a, bool active) {
+    dft32_perm_in<DIR>(x);
+#pragma unroll
+    for (int k2 = 1; k2 < NB; ++k2) {
+        cd w = tw[a * XS + k2];
+        if (DIR > 0) w = conj(w);
+        x[k2] = x[k2] * w;
+    }
+    if (active)
+#pragma unroll
+        for (int k2 = 0; k2 < NB; ++k2) buf[a * XS + k2] = x[k2];
+}
+// p2s, lane tau < 32: load column tau, DFT-24 -> x[0..23] (S layout)
+template <int DIR> NSC_HD void p2s_back(cd* x, const cd* buf, int tau) {
+#pragma unroll
+    for (int aa = 0; aa < NA; ++aa) x[aa] = buf[aa * XS + tau];
+    Dft<24, DIR>::run(x);
+}
+
+#ifdef __CUDACC__
+// Whole transforms for one warp; x has 32 elements.  `buf` is the warp's private exchange matrix.
+template <int DIR> __device__ __forceinline__ void s2p(cd* x, cd* buf, const cd* tw, int tau) {
+    __syncwarp();                      // every lane has finished reading buf (previous transform)
+    s2p_front<DIR>(x, buf, tw, tau);
+    __syncwarp();
+    s2p_back<DIR>(x, buf, tau < NA ? tau : NA - 1);
+}
+template <int DIR> __device__ __forceinline__ void p2s(cd* x, cd* buf, const cd* tw, int tau) {
+    __syncwarp();
+    p2s_front<DIR>(x, buf, tw, tau < NA ? tau : NA - 1, tau < NA);
+    __syncwarp();
+    p2s_back<DIR>(x, buf, tau);
+}
+
+// cooperative copy of the [24][33] twiddle matrix (global, plan.cu) into shared memory
+__device__ __forceinline__ void load_twiddles(cd* tw_s, const cd* tw_g) {
+    for (int i = threadIdx.x; i < XBUF; i += blockDim.x) tw_s[i] = tw_g[i];
+}
+#endif
+
+}  // namespace f768
+}  // namespace nsc

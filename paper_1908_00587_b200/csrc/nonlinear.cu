@@ -1,6 +1,6 @@
 // nonlinear.cu -- host driver of the nonlinear term N(u, T) (DESIGN.md steps N1-N6;
 // BASELINE.json north_star (a)): per radial chunk  k_zinv -> k_theta -> k_zfwd.
-#include "nonlinear_kernels.cuh"
+#include "nonlinear_v2_args.h"
 
 namespace nsc {
 
@@ -49,20 +49,57 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
     a.nf = c->nf;
     a.scale = 1.0 / ((double)c->Nt * (double)c->Nz);
     a.buoy = c->heated ? c->p.Ra / c->p.Pr : 0.0;
+    Nl2Args a2{};
+    a2.tw768 = c->t.tw768;
+    a2.alpha = c->p.alpha;
+    a2.ktheta0 = (double)c->p.k_theta0;
+    if (c->z768) {
+        // N1: D1 f of every field, once per evaluation (marching kernel)
+        DrArgs d{};
+        for (int i = 0; i < c->nf; ++i) {
+            d.f[i] = f[i];
+            d.out[i] = c->DR[i];
+            a2.dr[i] = c->DR[i];
+        }
+        d.D1 = c->t.D1;
+        d.N_r = c->N_r;
+        d.plane = (size_t)c->M1 * c->NK;
+        prof_begin(c, NSC_K_DR);
+        if (int e = launch_dr(d, c->nf, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_dr launch");
+        prof_end(c);
+    }
     for (int j0 = 0; j0 < c->N_r; j0 += c->JC) {
         a.j0 = j0;
         a.nj = (c->N_r - j0 < c->JC) ? c->N_r - j0 : c->JC;
         a.tw = c->t.tw_z;
         prof_begin(c, NSC_K_ZINV);
-        if (int e = lz->zinv(a, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zinv launch");
+        if (c->z768) {
+            a2.b = a;
+            a2.nitems = c->nf * a.nj * (c->MP / 4);
+            if (int e = launch_zinv2(a2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zinv2 launch");
+        } else if (int e = lz->zinv(a, c->stream)) {
+            return cuda_fail(c, (cudaError_t)e, "k_zinv launch");
+        }
         prof_end(c);
         a.tw = c->t.tw_t;
         prof_begin(c, NSC_K_THETA);
-        if (int e = lt->theta(a, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_theta launch");
+        if (c->t768) {
+            a2.b = a;
+            a2.nitems = a.nj * a.Nz;
+            if (int e = launch_theta2(a2, c->t768 == 2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_theta2 launch");
+        } else if (int e = lt->theta(a, c->stream)) {
+            return cuda_fail(c, (cudaError_t)e, "k_theta launch");
+        }
         prof_end(c);
         a.tw = c->t.tw_z;
         prof_begin(c, NSC_K_ZFWD);
-        if (int e = lz->zfwd(a, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zfwd launch");
+        if (c->z768) {
+            a2.b = a;
+            a2.nitems = c->nf * a.nj * (c->MP / 4);
+            if (int e = launch_zfwd2(a2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zfwd2 launch");
+        } else if (int e = lz->zfwd(a, c->stream)) {
+            return cuda_fail(c, (cudaError_t)e, "k_zfwd launch");
+        }
         prof_end(c);
     }
     return NSC_OK;

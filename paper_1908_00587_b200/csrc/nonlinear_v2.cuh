@@ -1,0 +1,621 @@
+// nonlinear_v2.cuh -- transform kernels of the nonlinear term specialised for line length 768
+// (BASELINE.json configs[3], the headline workload: 3/2-padded 768 x 768 grid per radial node).
+// Same steps N1-N6 and the same intermediate layout as nonlinear_kernels.cuh; what changes:
+//
+//   * the two-pass 24 x 32 transform of fft768.cuh: one shared-memory exchange per line instead of
+//     two, conflict-free, one warp per line and only warp-level barriers inside a transform;
+//   * k_dr     the radial derivative D1 f (N1) is taken once per evaluation by a marching kernel
+//              (one thread per (m, k) column, nine levels in registers), so that no transform
+//              kernel re-reads nine radial neighbours per line;
+//   * k_zinv2  four adjacent m-lines per CTA; the transposed [z][m] stores go through a swizzled
+//              shared-memory tile and leave as full 64-byte segments;
+//   * k_theta2 one (j, z) point-line per warp, the 12 real physical-space lines exist only in
+//              registers; the three velocity lines and one parked line live in a lane-private
+//              scratch -- Tensor Memory (tcgen05.st / tcgen05.ld, 256 columns per warp: TMEM as
+//              a 256 KB lane-private register spill space next to the 64 K registers) or shared
+//              memory (fallback variant);
+//   * k_zfwd2  cp.async double-buffered [z][4 m] tiles, forward transform, truncation, scaling,
+//              buoyancy.
+#pragma once
+#include <cstdint>
+#include "fft768.cuh"
+#include "nonlinear_v2_args.h"
+
+namespace nsc {
+
+
+// ------------------------------------------------------------------------------------------ k_dr
+// out[j] = sum_l D1[j][l] f[s0(j) + l],  s0(j) = clamp(j - 4, 0, N_r - 9)   (O2, R3)
+constexpr int DR_LA = 3;   // levels loaded ahead of the window (memory-level parallelism)
+__global__ void __launch_bounds__(128) k_dr(DrArgs a) {
+    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= a.plane) return;
+    const cd* src = a.f[blockIdx.y] + col;
+    cd* dst = a.out[blockIdx.y] + col;
+    const int N = a.N_r;
+    cd w[NPT + DR_LA];
+#pragma unroll
+    for (int l = 0; l < NPT + DR_LA; ++l) w[l] = (l < N) ? src[(size_t)l * a.plane] : mk(0.0, 0.0);
+    for (int j = 0; j < N; ++j) {
+        if (j > NPT / 2 && j <= N - 1 - NPT / 2) {   // the window start advanced by one level
+#pragma unroll
+            for (int l = 0; l < NPT + DR_LA - 1; ++l) w[l] = w[l + 1];
+            const int nxt = j - NPT / 2 + NPT - 1 + DR_LA;
+            w[NPT + DR_LA - 1] = (nxt < N) ? src[(size_t)nxt * a.plane] : mk(0.0, 0.0);
+        }
+        const double* d = a.D1 + j * NPT;
+        cd acc = mk(0.0, 0.0);
+#pragma unroll
+        for (int l = 0; l < NPT; ++l) {
+            const double c = __ldg(d + l);
+            acc.x = fma(c, w[l].x, acc.x);
+            acc.y = fma(c, w[l].y, acc.y);
+        }
+        dst[(size_t)j * a.plane] = acc;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+
+// swizzled position (in 16-byte chunks) of (z, m_local) in a [768][4] tile: conflict free both for
+// lanes walking z (transform side) and for lanes walking (z, m_local) row-major (global side)
+__device__ __forceinline__ int tile4(int z, int ml) { return z * 4 + (ml ^ ((z >> 1) & 3)); }
+
+// axial mode index kk = k + K of padded-line index i (i <= K or i >= 768 - K), and k as a double
+struct ZBin {
+    int kk;
+    double kd;
+    bool ok;
+};
+__device__ __forceinline__ ZBin z_bin(int i, int K) {
+    ZBin b;
+    if (i <= K) {
+        b.kk = i + K;
+        b.kd = (double)i;
+        b.ok = true;
+    } else if (i >= f768::N - K) {
+        b.kk = i - f768::N + K;
+        b.kd = (double)(i - f768::N);
+        b.ok = true;
+    } else {
+        b.kk = 0;
+        b.kd = 0.0;
+        b.ok = false;
+    }
+    return b;
+}
+
+// S-layout slots that can hold non-zero spectral data when the mode count is <= 256 = 768 / 3:
+// t = 0..8 (bins 0..287) and t = 16..23 (bins 512..767); t = 9..15 is always zero padding.
+#define NSC_S_SLOTS(OP) OP(0) OP(1) OP(2) OP(3) OP(4) OP(5) OP(6) OP(7) OP(8) OP(16) OP(17) OP(18) OP(19) OP(20) OP(21) OP(22) OP(23)
+
+constexpr int Z2_WARPS = 4;
+constexpr int Z2_THREADS = Z2_WARPS * 32;
+constexpr size_t Z2_SMEM_INV = sizeof(cd) * (size_t)(f768::XBUF * (1 + Z2_WARPS));
+constexpr size_t Z2_TILE = (size_t)f768::N * Z2_WARPS;                 // complex elements of one tile
+constexpr size_t Z2_SMEM_FWD = Z2_SMEM_INV + sizeof(cd) * Z2_TILE;     // + the second tile buffer
+
+// ------------------------------------------------------------------------------------------ k_zinv2
+// work item = (field, level, tile of 4 adjacent m); three inverse transforms per line:
+// q = 1 (i kappa f), q = 0 (f), q = 2 (D1 f).
+__global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
+    using namespace f768;
+    const NlArgs& a = A.b;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cd* tw = reinterpret_cast<cd*>(smem_raw);
+    cd* tile = tw + XBUF;                               // [768][4] tile, overlays the 4 matrices
+    const int warp = threadIdx.x >> 5, tau = threadIdx.x & 31;
+    cd* buf = tile + warp * XBUF;
+    load_twiddles(tw, A.tw768);
+    __syncthreads();
+    const int a23 = tau < NA ? tau : NA - 1;
+    const int mtiles = a.MP / 4;
+    const size_t plane = (size_t)a.M1 * a.NK;
+    const size_t qstride = (size_t)a.JC * N * a.MP;
+    const double taud = (double)tau;
+
+    int item = blockIdx.x;
+    cd F[17];
+    // loads the 17 potentially non-zero S-layout slots of one spectral line
+    auto load_line = [&](const cd* base, int it, cd* dst) {
+        const int mt = it % mtiles, r = it / mtiles;
+        const int jl = r % a.nj, fi = r / a.nj;
+        const int m = mt * 4 + warp;
+        const bool vm = (it < A.nitems) && (m < a.M1);
+        const cd* src = base + (size_t)(a.j0 + jl) * plane + (size_t)(vm ? m : 0) * a.NK;
+        (void)fi;
+        int s = 0;
+#define NSC_LD(T)                                                  \
+    {                                                              \
+        ZBin zb = z_bin(tau + 32 * T, a.K);                        \
+        dst[s] = (vm && zb.ok) ? src[zb.kk] : mk(0.0, 0.0);        \
+        ++s;                                                       \
+    }
+        NSC_S_SLOTS(NSC_LD)
+#undef NSC_LD
+    };
+    auto field_of = [&](int it) { return (it / mtiles) / a.nj; };
+    if (item < A.nitems) load_line(a.f[field_of(item)], item, F);
+
+    for (; item < A.nitems; item += gridDim.x) {
+        const int mt = item % mtiles, r = item / mtiles;
+        const int jl = r % a.nj, fi = r / a.nj;
+        cd x[32];
+        // stores the P-layout result of this warp's line into the tile and writes the tile out
+        auto emit = [&](int q) {
+            __syncthreads();                            // all warps left their exchange matrices
+            if (tau < NA) {
+#pragma unroll
+                for (int e = 0; e < 32; ++e) tile[tile4(p_idx(e, tau), warp)] = x[e];
+            }
+            __syncthreads();
+            cd* dst = a.zbuf + (size_t)(3 * fi + q) * qstride + (size_t)jl * N * a.MP + mt * 4;
+#pragma unroll 4
+            for (int it = 0; it < (N * 4) / Z2_THREADS; ++it) {
+                const int id = threadIdx.x + it * Z2_THREADS;
+                const int z = id >> 2, c = id & 3;
+                dst[(size_t)z * a.MP + (c ^ ((z >> 1) & 3))] = tile[id];
+            }
+            __syncthreads();                            // tile free again
+        };
+        // ---- q = 1: i kappa f
+        {
+            int s = 0;
+#define NSC_SET(T)                                                       \
+    {                                                                    \
+        const double kd = (T <= 8) ? taud + (double)(32 * T) : taud + (double)(32 * T - N); \
+        x[T] = (A.alpha * kd) * mul_i(F[s]);                             \
+        ++s;                                                             \
+    }
+            NSC_S_SLOTS(NSC_SET)
+#undef NSC_SET
+#pragma unroll
+            for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
+        }
+        s2p<+1>(x, buf, tw, tau);
+        emit(1);
+        // ---- q = 0: f  (F dies here); the D1 f line is requested before the transform
+        {
+            int s = 0;
+#define NSC_SET(T) \
+    {              \
+        x[T] = F[s]; \
+        ++s;       \
+    }
+            NSC_S_SLOTS(NSC_SET)
+#undef NSC_SET
+#pragma unroll
+            for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
+        }
+        cd D[17];
+        load_line(A.dr[fi], item, D);
+        s2p<+1>(x, buf, tw, tau);
+        emit(0);
+        // ---- q = 2: D1 f; the next item's f line is requested before the transform
+        {
+            int s = 0;
+#define NSC_SET(T) \
+    {              \
+        x[T] = D[s]; \
+        ++s;       \
+    }
+            NSC_S_SLOTS(NSC_SET)
+#undef NSC_SET
+#pragma unroll
+            for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
+        }
+        const int nxt = item + gridDim.x;
+        if (nxt < A.nitems) load_line(a.f[field_of(nxt)], nxt, F);
+        s2p<+1>(x, buf, tw, tau);
+        emit(2);
+    }
+    (void)a23;
+}
+
+// ------------------------------------------------------------------------------------------ k_zfwd2
+// work item = (field, level, tile of 4 adjacent m).  The [768][4] tile of theta-transformed
+// products arrives by cp.async (64-byte segments) while the previous item is being transformed.
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit_wait_all() {
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
+__global__ void __launch_bounds__(Z2_THREADS, 2) k_zfwd2(Nl2Args A) {
+    using namespace f768;
+    const NlArgs& a = A.b;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cd* tw = reinterpret_cast<cd*>(smem_raw);
+    const int warp = threadIdx.x >> 5, tau = threadIdx.x & 31;
+    cd* buf = tw + XBUF + warp * XBUF;
+    cd* tile = tw + XBUF * (1 + Z2_WARPS);
+    load_twiddles(tw, A.tw768);
+    const int a23 = tau < NA ? tau : NA - 1;
+    const int mtiles = a.MP / 4;
+    const size_t qstride = (size_t)a.JC * N * a.MP;
+
+    auto fetch = [&](int it) {
+        const int mt = it % mtiles, r = it / mtiles;
+        const int jl = r % a.nj, fi = r / a.nj;
+        const cd* src = a.tbuf + (size_t)fi * qstride + (size_t)jl * N * a.MP + mt * 4;
+#pragma unroll 4
+        for (int k = 0; k < (N * 4) / Z2_THREADS; ++k) {
+            const int id = threadIdx.x + k * Z2_THREADS;
+            const int z = id >> 2, c = id & 3;
+            cp_async16(tile + id, src + (size_t)z * a.MP + (c ^ ((z >> 1) & 3)));
+        }
+    };
+    int item = blockIdx.x;
+    if (item < A.nitems) fetch(item);
+    for (; item < A.nitems; item += gridDim.x) {
+        const int mt = item % mtiles, r = item / mtiles;
+        const int jl = r % a.nj, fi = r / a.nj;
+        const int j = a.j0 + jl, m = mt * 4 + warp;
+        cp_async_commit_wait_all();
+        __syncthreads();                                 // the tile (and, first time, tw) is complete
+        cd x[32];
+#pragma unroll
+        for (int e = 0; e < 32; ++e) x[e] = tile[tile4(p_idx(e, a23), warp)];
+        __syncthreads();                                 // every warp holds its line: the tile is free
+        if (item + (int)gridDim.x < A.nitems) fetch(item + gridDim.x);
+        p2s<-1>(x, buf, tw, tau);
+        if (m < a.M1) {
+            const size_t off = ((size_t)j * a.M1 + m) * a.NK;
+            cd* dst = a.out[fi] + off;
+            const bool add_buoy = (fi == 2) && (a.buoy != 0.0);
+            const cd* Th = a.f[add_buoy ? 3 : 0] + off;
+#define NSC_ST(T)                                          \
+    {                                                      \
+        ZBin zb = z_bin(tau + 32 * T, a.K);                \
+        if (zb.ok) {                                       \
+            cd v = a.scale * x[T];                         \
+            if (add_buoy) {                                \
+                cd th = Th[zb.kk];                         \
+                v.x = fma(a.buoy, th.x, v.x);              \
+                v.y = fma(a.buoy, th.y, v.y);              \
+            }                                              \
+            dst[zb.kk] = v;                                \
+        }                                                  \
+    }
+            NSC_S_SLOTS(NSC_ST)
+#undef NSC_ST
+        }
+    }
+    cp_async_commit_wait_all();
+}
+
+// ------------------------------------------------------------------------------------------ scratch
+// Lane-private scratch of k_theta2: NSLOT lines of 32 doubles per lane.  Two implementations with
+// the same interface: st(slot, v[32]) / ld(slot, v[32]), both warp-collective.
+constexpr int T2_NSLOT = 4;            // U_r, U_theta / r, U_z, one parked line
+
+// (1) Tensor Memory.  A CTA of 8 warps owns all 512 columns of its SM's TMEM; warp w may touch the
+// 32 lanes of its quadrant (w & 3) only, so warps w and w + 4 share lanes and split the columns:
+// 256 columns = 128 doubles per thread = 4 slots of 32.  tcgen05.st / .ld with shape 32x32b move one
+// 32-bit column per register per lane; x16 = 8 doubles per instruction.
+struct TmemScratch {
+    uint32_t base;        // TMEM address (lane << 16 | column) of this warp's slot 0
+    __device__ __forceinline__ void st8(uint32_t addr, const double* v) const {
+        asm volatile(
+            "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, "
+            "%14, %15, %16};" ::"r"(addr),
+            "r"(__double2loint(v[0])), "r"(__double2hiint(v[0])), "r"(__double2loint(v[1])),
+            "r"(__double2hiint(v[1])), "r"(__double2loint(v[2])), "r"(__double2hiint(v[2])),
+            "r"(__double2loint(v[3])), "r"(__double2hiint(v[3])), "r"(__double2loint(v[4])),
+            "r"(__double2hiint(v[4])), "r"(__double2loint(v[5])), "r"(__double2hiint(v[5])),
+            "r"(__double2loint(v[6])), "r"(__double2hiint(v[6])), "r"(__double2loint(v[7])),
+            "r"(__double2hiint(v[7]))
+            : "memory");
+    }
+    __device__ __forceinline__ void ld8(uint32_t addr, double* v) const {
+        uint32_t r[16];
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, "
+            "%14, %15}, [%16];"
+            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+              "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+            : "r"(addr)
+            : "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = __hiloint2double((int)r[2 * i + 1], (int)r[2 * i]);
+    }
+    __device__ __forceinline__ void st(int slot, const double* v) const {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) st8(base + slot * 64 + c * 16, v + 8 * c);
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+    __device__ __forceinline__ void ld(int slot, double* v) const {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) ld8(base + slot * 64 + c * 16, v + 8 * c);
+    }
+};
+
+// (2) shared memory: [slot][e][24 lanes] doubles per warp (lanes >= 24 hold nothing)
+struct SmemScratch {
+    double* base;         // this warp's block of T2_NSLOT * 32 * 24 doubles, already offset by the lane
+    bool active;
+    __device__ __forceinline__ void st(int slot, const double* v) const {
+        if (active)
+#pragma unroll
+            for (int e = 0; e < 32; ++e) base[(slot * 32 + e) * f768::NA] = v[e];
+    }
+    __device__ __forceinline__ void ld(int slot, double* v) const {
+#pragma unroll
+        for (int e = 0; e < 32; ++e) v[e] = base[(slot * 32 + e) * f768::NA];
+    }
+};
+
+template <bool TMEM> struct T2Cfg;
+template <> struct T2Cfg<true> {
+    static constexpr int WARPS = 8;
+    using Scratch = TmemScratch;
+    // the request is padded above half of the SM's shared memory so that exactly one CTA (the owner
+    // of all 512 TMEM columns) is resident per SM
+    static constexpr size_t SMEM = 120 * 1024;
+};
+template <> struct T2Cfg<false> {
+    static constexpr int WARPS = 5;
+    using Scratch = SmemScratch;
+    static constexpr size_t SMEM =
+        sizeof(cd) * (size_t)f768::XBUF * (1 + WARPS) + sizeof(double) * (size_t)WARPS * T2_NSLOT * 32 * f768::NA;
+};
+
+// chunked access (8 doubles = elements 8 c .. 8 c + 7 of a slot)
+__device__ __forceinline__ void sc_st8(const TmemScratch& s, int slot, int c, const double* v) {
+    s.st8(s.base + slot * 64 + c * 16, v);
+}
+__device__ __forceinline__ void sc_ld8(const TmemScratch& s, int slot, int c, double* v) {
+    s.ld8(s.base + slot * 64 + c * 16, v);
+}
+__device__ __forceinline__ void sc_fence(const TmemScratch&) {
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void sc_st8(const SmemScratch& s, int slot, int c, const double* v) {
+    if (s.active)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) s.base[(slot * 32 + c * 8 + i) * f768::NA] = v[i];
+}
+__device__ __forceinline__ void sc_ld8(const SmemScratch& s, int slot, int c, double* v) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = s.base[(slot * 32 + c * 8 + i) * f768::NA];
+}
+__device__ __forceinline__ void sc_fence(const SmemScratch&) {}
+
+// ------------------------------------------------------------------------------------------ k_theta2
+// Z[i] = G_X(i) + i G_Y(i) in the S layout, G(m) = mult * line[m] (0 <= m <= M), G(-m) = conj G(m),
+// Im G(0) dropped (R6); mult = 1 or i n_m (d/dtheta, N1).  Slots t = 9..15 are zero padding.
+template <bool DX, bool DY, bool HAS_Y>
+__device__ __forceinline__ void load_pair768(cd* x, const cd* X, const cd* Y, int M, int tau, double taud,
+                                             double kth0) {
+#define NSC_POS(T)                                                    \
+    {                                                                 \
+        const int m = tau + 32 * T;                                   \
+        const bool ok = m <= M;                                       \
+        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
+        cd gy = (HAS_Y && ok) ? Y[m] : mk(0.0, 0.0);                  \
+        const double n = kth0 * (taud + (double)(32 * T));            \
+        if (DX) gx = n * mul_i(gx);                                   \
+        if (DY) gy = n * mul_i(gy);                                   \
+        if (T == 0 && tau == 0) {                                     \
+            gx.y = 0.0;                                               \
+            gy.y = 0.0;                                               \
+        }                                                             \
+        x[T] = mk(gx.x - gy.y, gx.y + gy.x);                          \
+    }
+#define NSC_NEG(T)                                                    \
+    {                                                                 \
+        const int m = f768::N - 32 * T - tau;                         \
+        const bool ok = m <= M;                                       \
+        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
+        cd gy = (HAS_Y && ok) ? Y[m] : mk(0.0, 0.0);                  \
+        const double n = kth0 * ((double)(f768::N - 32 * T) - taud);  \
+        if (DX) gx = n * mul_i(gx);                                   \
+        if (DY) gy = n * mul_i(gy);                                   \
+        x[T] = mk(gx.x + gy.y, gy.x - gx.y);                          \
+    }
+    NSC_POS(0) NSC_POS(1) NSC_POS(2) NSC_POS(3) NSC_POS(4) NSC_POS(5) NSC_POS(6) NSC_POS(7) NSC_POS(8)
+#pragma unroll
+    for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
+    NSC_NEG(16) NSC_NEG(17) NSC_NEG(18) NSC_NEG(19) NSC_NEG(20) NSC_NEG(21) NSC_NEG(22) NSC_NEG(23)
+#undef NSC_POS
+#undef NSC_NEG
+}
+
+// Splits the forward transform Z (S layout) of a packed real pair (a + i b) into the Hermitian half
+// lines A[m] = (Z[m] + conj Z[N-m]) / 2, B[m] = (Z[m] - conj Z[N-m]) / (2 i), m <= M (N5 truncation).
+// Z[N-m] of lane tau, slot T sits in lane (32 - tau) & 31, slot 23 - T (lane 0: its own slot 24 - T).
+template <bool HAS_B>
+__device__ __forceinline__ void store_pair768(const cd* x, cd* outA, cd* outB, int M, int tau) {
+    const int src = (32 - tau) & 31;
+#define NSC_OUT(T)                                                                 \
+    {                                                                              \
+        cd pz;                                                                     \
+        if (T == 8) {                                                              \
+            pz = x[16];                                                            \
+        } else {                                                                   \
+            pz.x = __shfl_sync(0xffffffffu, x[23 - T].x, src);                     \
+            pz.y = __shfl_sync(0xffffffffu, x[23 - T].y, src);                     \
+            if (tau == 0) pz = (T == 0) ? x[0] : x[(24 - T) % 24];                 \
+        }                                                                          \
+        const int m = tau + 32 * T;                                                \
+        if (m <= M) {                                                              \
+            const cd zm = conj(pz);                                                \
+            outA[m] = 0.5 * (x[T] + zm);                                           \
+            if (HAS_B) outB[m] = 0.5 * mul_mi(x[T] - zm);                          \
+        }                                                                          \
+    }
+    NSC_OUT(0) NSC_OUT(1) NSC_OUT(2) NSC_OUT(3) NSC_OUT(4) NSC_OUT(5) NSC_OUT(6) NSC_OUT(7) NSC_OUT(8)
+#undef NSC_OUT
+}
+
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+template <bool TMEM>
+__global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A) {
+    using namespace f768;
+    using Cfg = T2Cfg<TMEM>;
+    const NlArgs& a = A.b;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t tmem_base_s;
+    cd* tw = reinterpret_cast<cd*>(smem_raw);
+    const int warp = threadIdx.x >> 5, tau = threadIdx.x & 31;
+    cd* buf = tw + XBUF * (1 + warp);
+    const int a23 = tau < NA ? tau : NA - 1;
+    load_twiddles(tw, A.tw768);
+    typename Cfg::Scratch sc;
+    if constexpr (TMEM) {
+        if (warp == 0) {
+            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&tmem_base_s);
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(dst) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        sc.base = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 256);
+    } else {
+        double* sb = reinterpret_cast<double*>(tw + XBUF * (1 + Cfg::WARPS));
+        sc.base = sb + (size_t)warp * T2_NSLOT * 32 * NA + a23;
+        sc.active = tau < NA;
+        __syncthreads();
+    }
+    const int M = a.M;
+    const double taud = (double)tau, kth0 = A.ktheta0;
+    const size_t qstride = (size_t)a.JC * a.Nz * a.MP;
+    const int nlines = a.nj * a.Nz;
+    const int lstride = gridDim.x * Cfg::WARPS;
+#define LINE_A(f) (a.zbuf + (size_t)(3 * (f) + 0) * qstride + loff)
+#define LINE_B(f) (a.zbuf + (size_t)(3 * (f) + 1) * qstride + loff)
+#define LINE_C(f) (a.zbuf + (size_t)(3 * (f) + 2) * qstride + loff)
+#define LINE_O(f) (a.tbuf + (size_t)(f) * qstride + loff)
+    for (int line = blockIdx.x * Cfg::WARPS + warp; line < nlines; line += lstride) {
+        const int jl = line / a.Nz;
+        const size_t loff = (size_t)line * a.MP;               // (jl * Nz + z) * MP
+        const double ri = a.rinv[a.j0 + jl];
+        const double rj = 1.0 / ri;
+        if (line + lstride < nlines) {                         // next line's nine inputs -> L2
+            const size_t noff = (size_t)(line + lstride) * a.MP;
+#pragma unroll
+            for (int q = 0; q < 9; ++q) {
+                const char* p = reinterpret_cast<const char*>(a.zbuf + (size_t)q * qstride + noff);
+                prefetch_l2(p + tau * 128);
+                if (tau == 0) prefetch_l2(p + 32 * 128);
+            }
+        }
+        cd x[32];
+        double acc[32];
+        double t0[8], t1[8], t2[8];
+        // T1: (u_r, u_theta) -> slots 0 (U_r), 1 (U_theta / r)
+        load_pair768<false, false, true>(x, LINE_A(0), LINE_A(1), M, tau, taud, kth0);
+        s2p<+1>(x, buf, tw, tau);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                t0[i] = x[8 * c + i].x;
+                t1[i] = x[8 * c + i].y * ri;
+            }
+            sc_st8(sc, 0, c, t0);
+            sc_st8(sc, 1, c, t1);
+        }
+        // T2: (u_z, d_r u_r) -> slot 2 (U_z); acc = U_r d_r u_r
+        load_pair768<false, false, true>(x, LINE_A(2), LINE_C(0), M, tau, taud, kth0);
+        s2p<+1>(x, buf, tw, tau);
+        sc_fence(sc);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            sc_ld8(sc, 0, c, t0);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                t2[i] = x[8 * c + i].x;
+                acc[8 * c + i] = t0[i] * x[8 * c + i].y;
+            }
+            sc_st8(sc, 2, c, t2);
+        }
+        // T3: (d_theta u_r, d_z u_r);  N_r = -(u.grad u_r - u_theta^2 / r) -> slot 3
+        load_pair768<true, false, true>(x, LINE_A(0), LINE_B(0), M, tau, taud, kth0);
+        s2p<+1>(x, buf, tw, tau);
+        sc_fence(sc);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            sc_ld8(sc, 1, c, t1);
+            sc_ld8(sc, 2, c, t2);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                double s = fma(t1[i], x[8 * c + i].x, acc[8 * c + i]);
+                s = fma(t2[i], x[8 * c + i].y, s);
+                s = fma(-(t1[i] * rj), t1[i], s);
+                t0[i] = -s;
+            }
+            sc_st8(sc, 3, c, t0);
+        }
+        // T4: (d_r u_theta, d_theta u_theta)
+        load_pair768<false, true, true>(x, LINE_C(1), LINE_A(1), M, tau, taud, kth0);
+        s2p<+1>(x, buf, tw, tau);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            sc_ld8(sc, 0, c, t0);
+            sc_ld8(sc, 1, c, t1);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) acc[8 * c + i] = fma(t1[i], x[8 * c + i].y, t0[i] * x[8 * c + i].x);
+        }
+        // T5: (d_z u_theta, d_r u_z);  N_theta = -(u.grad u_theta + u_r u_theta / r);
+        //     slot 3: N_r out, U_r d_r u_z in;  x <- (N_r, N_theta)
+        load_pair768<false, false, true>(x, LINE_B(1), LINE_C(2), M, tau, taud, kth0);
+        s2p<+1>(x, buf, tw, tau);
+        sc_fence(sc);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            double t3[8];
+            sc_ld8(sc, 0, c, t0);
+            sc_ld8(sc, 1, c, t1);
+            sc_ld8(sc, 2, c, t2);
+            sc_ld8(sc, 3, c, t3);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                double s = fma(t2[i], x[8 * c + i].x, acc[8 * c + i]);
+                s = fma(t0[i], t1[i], s);
+                t2[i] = t0[i] * x[8 * c + i].y;
+                x[8 * c + i] = mk(t3[i], -s);
+            }
+            sc_st8(sc, 3, c, t2);
+        }
+        p2s<-1>(x, buf, tw, tau);
+        store_pair768<true>(x, LINE_O(0), LINE_O(1), M, tau);
+        // T6: (d_theta u_z, d_z u_z);  N_z = -(u.grad u_z)   (buoyancy is added in k_zfwd)
+        load_pair768<true, false, true>(x, LINE_A(2), LINE_B(2), M, tau, taud, kth0);
+        s2p<+1>(x, buf, tw, tau);
+        sc_fence(sc);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            sc_ld8(sc, 1, c, t1);
+            sc_ld8(sc, 2, c, t2);
+            sc_ld8(sc, 3, c, t0);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                double s = fma(t1[i], x[8 * c + i].x, t0[i]);
+                s = fma(t2[i], x[8 * c + i].y, s);
+                x[8 * c + i] = mk(-s, 0.0);
+            }
+        }
+        p2s<-1>(x, buf, tw, tau);
+        store_pair768<false>(x, LINE_O(2), nullptr, M, tau);
+    }
+#undef LINE_A
+#undef LINE_B
+#undef LINE_C
+#undef LINE_O
+    if constexpr (TMEM) {
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (warp == 0)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base_s) : "memory");
+    }
+}
+
+}  // namespace nsc

@@ -43,6 +43,7 @@ struct Tables {               // all device pointers
     double* kap = nullptr;    // [2K+1]     kappa = k alpha
     cd* tw_t = nullptr;       // [N_theta]  exp(-2 pi i t / N_theta)
     cd* tw_z = nullptr;       // [N_z]
+    cd* tw768 = nullptr;      // [24][33]   exp(-2 pi i k1 n2 / 768) of fft768.cuh (if a length is 768)
 };
 
 }  // namespace nsc
@@ -63,6 +64,9 @@ struct nsc_ctx {
     nsc::cd* N1[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* zbuf = nullptr;              // [3 nf][JC][N_z][MP]  z-transformed f, dz f, dr f
     nsc::cd* tbuf = nullptr;              // [nf][JC][N_z][MP]    theta-transformed products
+    nsc::cd* DR[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};       // D1 f (length-768 z pipeline)
+    bool z768 = false;                    // z transforms by k_dr + k_zinv2 / k_zfwd2
+    int t768 = 0;                         // theta transforms by k_theta2: 0 no, 1 shared-memory, 2 TMEM scratch
     nsc::BandShape shH, shP;              // Helmholtz (9-wide rows) / Poisson (17-wide rows) envelopes
     nsc::BandFactors facH[4];             // u_+, u_-, u_z, T
     nsc::BandFactors facP;

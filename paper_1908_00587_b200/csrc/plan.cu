@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstring>
 #include "nsc_internal.h"
+#include "fft768.cuh"
 
 namespace nsc {
 
@@ -160,6 +161,16 @@ int build_plan(nsc_ctx* c) {
     if ((rc = upload(c, &c->t.kap, kap))) return rc;
     if ((rc = upload(c, &c->t.tw_t, twiddles(c->Nt)))) return rc;
     if ((rc = upload(c, &c->t.tw_z, twiddles(c->Nz)))) return rc;
+    if (c->Nt == f768::N || c->Nz == f768::N) {
+        // exp(-2 pi i k1 n2 / 768), k1 < 24, n2 < 32, row stride 33 (fft768.cuh)
+        std::vector<cd> t(f768::XBUF, mk(0.0, 0.0));
+        for (int k1 = 0; k1 < f768::NA; ++k1)
+            for (int n2 = 0; n2 < f768::NB; ++n2) {
+                ld a = 2 * pi_ld() * (ld)(k1 * n2) / f768::N;
+                t[k1 * f768::XS + n2] = mk((double)cosl(a), (double)(-sinl(a)));
+            }
+        if ((rc = upload(c, &c->t.tw768, t))) return rc;
+    }
 
     // ---- band envelopes.  Helmholtz: identity rows at the walls (Dirichlet), stencil rows inside.
     c->shH.h_lo.resize(N);

@@ -23,7 +23,7 @@ EXPORTS = (
     "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_last_error", "nsc_device_bytes",
     "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name",
 )
-NSC_NKERN = 10
+NSC_NKERN = 11
 
 NSC_OK, NSC_EINVAL, NSC_ENOMEM, NSC_ECUDA, NSC_ESTATE = 0, -1, -2, -3, -4
 
