@@ -451,9 +451,76 @@ __device__ __forceinline__ void store_pair768(const cd* x, cd* outA, cd* outB, i
 #undef NSC_OUT
 }
 
+__device__ __forceinline__ void store_pair768_rt(const cd* x, cd* outA, cd* outB, bool HAS_B, int M, int tau) {
+    const int src = (32 - tau) & 31;
+#define NSC_OUT(T)                                                                 \
+    {                                                                              \
+        cd pz;                                                                     \
+        if (T == 8) {                                                              \
+            pz = x[16];                                                            \
+        } else {                                                                   \
+            pz.x = __shfl_sync(0xffffffffu, x[23 - T].x, src);                     \
+            pz.y = __shfl_sync(0xffffffffu, x[23 - T].y, src);                     \
+            if (tau == 0) pz = (T == 0) ? x[0] : x[(24 - T) % 24];                 \
+        }                                                                          \
+        const int m = tau + 32 * T;                                                \
+        if (m <= M) {                                                              \
+            const cd zm = conj(pz);                                                \
+            outA[m] = 0.5 * (x[T] + zm);                                           \
+            if (HAS_B) outB[m] = 0.5 * mul_mi(x[T] - zm);                          \
+        }                                                                          \
+    }
+    NSC_OUT(0) NSC_OUT(1) NSC_OUT(2) NSC_OUT(3) NSC_OUT(4) NSC_OUT(5) NSC_OUT(6) NSC_OUT(7) NSC_OUT(8)
+#undef NSC_OUT
+}
+
 __device__ __forceinline__ void prefetch_l2(const void* p) {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
+
+// run-time variant of load_pair768 (dx, dy select the d/dtheta multiplier i n): one copy of the code
+// serves all six inverse transforms of a point-line, which keeps the kernel inside the instruction cache
+__device__ __forceinline__ void load_pair768_rt(cd* x, const cd* X, const cd* Y, bool dx, bool dy, int M, int tau,
+                                                double taud, double kth0) {
+#define NSC_POS(T)                                                    \
+    {                                                                 \
+        const int m = tau + 32 * T;                                   \
+        const bool ok = m <= M;                                       \
+        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
+        cd gy = ok ? Y[m] : mk(0.0, 0.0);                             \
+        const double n = kth0 * (taud + (double)(32 * T));            \
+        if (dx) gx = n * mul_i(gx);                                   \
+        if (dy) gy = n * mul_i(gy);                                   \
+        if (T == 0 && tau == 0) {                                     \
+            gx.y = 0.0;                                               \
+            gy.y = 0.0;                                               \
+        }                                                             \
+        x[T] = mk(gx.x - gy.y, gx.y + gy.x);                          \
+    }
+#define NSC_NEG(T)                                                    \
+    {                                                                 \
+        const int m = f768::N - 32 * T - tau;                         \
+        const bool ok = m <= M;                                       \
+        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
+        cd gy = ok ? Y[m] : mk(0.0, 0.0);                             \
+        const double n = kth0 * ((double)(f768::N - 32 * T) - taud);  \
+        if (dx) gx = n * mul_i(gx);                                   \
+        if (dy) gy = n * mul_i(gy);                                   \
+        x[T] = mk(gx.x + gy.y, gy.x - gx.y);                          \
+    }
+    NSC_POS(0) NSC_POS(1) NSC_POS(2) NSC_POS(3) NSC_POS(4) NSC_POS(5) NSC_POS(6) NSC_POS(7) NSC_POS(8)
+#pragma unroll
+    for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
+    NSC_NEG(16) NSC_NEG(17) NSC_NEG(18) NSC_NEG(19) NSC_NEG(20) NSC_NEG(21) NSC_NEG(22) NSC_NEG(23)
+#undef NSC_POS
+#undef NSC_NEG
+}
+
+// The six inverse transforms of a point-line as a table: work array index q = 3 field + kind
+// (kind 0 f, 1 d_z f, 2 d_r f) of the X and Y halves of the packed pair, d/dtheta flags.
+//   t : 0 (u_r, u_th)  1 (u_z, dr u_r)  2 (dth u_r, dz u_r)  3 (dr u_th, dth u_th)  4 (dz u_th, dr u_z)  5 (dth u_z, dz u_z)
+__device__ __forceinline__ int t2_qx(int t) { return (0x645060 >> (4 * t)) & 15; }
+__device__ __forceinline__ int t2_qy(int t) { return (0x783123 >> (4 * t)) & 15; }
 
 template <bool TMEM>
 __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A) {
@@ -489,10 +556,6 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
     const size_t qstride = (size_t)a.JC * a.Nz * a.MP;
     const int nlines = a.nj * a.Nz;
     const int lstride = gridDim.x * Cfg::WARPS;
-#define LINE_A(f) (a.zbuf + (size_t)(3 * (f) + 0) * qstride + loff)
-#define LINE_B(f) (a.zbuf + (size_t)(3 * (f) + 1) * qstride + loff)
-#define LINE_C(f) (a.zbuf + (size_t)(3 * (f) + 2) * qstride + loff)
-#define LINE_O(f) (a.tbuf + (size_t)(f) * qstride + loff)
     for (int line = blockIdx.x * Cfg::WARPS + warp; line < nlines; line += lstride) {
         const int jl = line / a.Nz;
         const size_t loff = (size_t)line * a.MP;               // (jl * Nz + z) * MP
@@ -509,107 +572,101 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
         }
         cd x[32];
         double acc[32];
-        double t0[8], t1[8], t2[8];
-        // T1: (u_r, u_theta) -> slots 0 (U_r), 1 (U_theta / r)
-        load_pair768<false, false, true>(x, LINE_A(0), LINE_A(1), M, tau, taud, kth0);
-        s2p<+1>(x, buf, tw, tau);
+#pragma unroll 1
+        for (int t = 0; t < 6; ++t) {
+            const cd* X = a.zbuf + (size_t)t2_qx(t) * qstride + loff;
+            const cd* Y = a.zbuf + (size_t)t2_qy(t) * qstride + loff;
+            load_pair768_rt(x, X, Y, t == 2 || t == 5, t == 3, M, tau, taud, kth0);
+            s2p<+1>(x, buf, tw, tau);
+            sc_fence(sc);
+            // physical-space stage (N4): slots 0 U_r, 1 U_theta / r, 2 U_z, 3 parked line
+            if (t == 0) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
+                for (int c = 0; c < 4; ++c) {
+                    double t0[8], t1[8];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                t0[i] = x[8 * c + i].x;
-                t1[i] = x[8 * c + i].y * ri;
+                    for (int i = 0; i < 8; ++i) {
+                        t0[i] = x[8 * c + i].x;
+                        t1[i] = x[8 * c + i].y * ri;
+                    }
+                    sc_st8(sc, 0, c, t0);
+                    sc_st8(sc, 1, c, t1);
+                }
+            } else if (t == 1) {                               // acc = U_r d_r u_r
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double t0[8], t2[8];
+                    sc_ld8(sc, 0, c, t0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        t2[i] = x[8 * c + i].x;
+                        acc[8 * c + i] = t0[i] * x[8 * c + i].y;
+                    }
+                    sc_st8(sc, 2, c, t2);
+                }
+            } else if (t == 2) {                               // N_r = -(u.grad u_r - u_theta^2 / r) -> slot 3
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double t0[8], t1[8], t2[8];
+                    sc_ld8(sc, 1, c, t1);
+                    sc_ld8(sc, 2, c, t2);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        double s = fma(t1[i], x[8 * c + i].x, acc[8 * c + i]);
+                        s = fma(t2[i], x[8 * c + i].y, s);
+                        s = fma(-(t1[i] * rj), t1[i], s);
+                        t0[i] = -s;
+                    }
+                    sc_st8(sc, 3, c, t0);
+                }
+            } else if (t == 3) {                               // acc = U_r d_r u_th + (U_th / r) d_th u_th
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double t0[8], t1[8];
+                    sc_ld8(sc, 0, c, t0);
+                    sc_ld8(sc, 1, c, t1);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) acc[8 * c + i] = fma(t1[i], x[8 * c + i].y, t0[i] * x[8 * c + i].x);
+                }
+            } else if (t == 4) {                               // N_theta; x <- (N_r, N_theta); slot 3 <- U_r d_r u_z
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double t0[8], t1[8], t2[8], t3[8];
+                    sc_ld8(sc, 0, c, t0);
+                    sc_ld8(sc, 1, c, t1);
+                    sc_ld8(sc, 2, c, t2);
+                    sc_ld8(sc, 3, c, t3);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        double s = fma(t2[i], x[8 * c + i].x, acc[8 * c + i]);
+                        s = fma(t0[i], t1[i], s);
+                        t2[i] = t0[i] * x[8 * c + i].y;
+                        x[8 * c + i] = mk(t3[i], -s);
+                    }
+                    sc_st8(sc, 3, c, t2);
+                }
+            } else {                                           // N_z = -(u.grad u_z)  (buoyancy: k_zfwd)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double t0[8], t1[8], t2[8];
+                    sc_ld8(sc, 1, c, t1);
+                    sc_ld8(sc, 2, c, t2);
+                    sc_ld8(sc, 3, c, t0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        double s = fma(t1[i], x[8 * c + i].x, t0[i]);
+                        s = fma(t2[i], x[8 * c + i].y, s);
+                        x[8 * c + i] = mk(-s, 0.0);
+                    }
+                }
             }
-            sc_st8(sc, 0, c, t0);
-            sc_st8(sc, 1, c, t1);
-        }
-        // T2: (u_z, d_r u_r) -> slot 2 (U_z); acc = U_r d_r u_r
-        load_pair768<false, false, true>(x, LINE_A(2), LINE_C(0), M, tau, taud, kth0);
-        s2p<+1>(x, buf, tw, tau);
-        sc_fence(sc);
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            sc_ld8(sc, 0, c, t0);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                t2[i] = x[8 * c + i].x;
-                acc[8 * c + i] = t0[i] * x[8 * c + i].y;
-            }
-            sc_st8(sc, 2, c, t2);
-        }
-        // T3: (d_theta u_r, d_z u_r);  N_r = -(u.grad u_r - u_theta^2 / r) -> slot 3
-        load_pair768<true, false, true>(x, LINE_A(0), LINE_B(0), M, tau, taud, kth0);
-        s2p<+1>(x, buf, tw, tau);
-        sc_fence(sc);
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            sc_ld8(sc, 1, c, t1);
-            sc_ld8(sc, 2, c, t2);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                double s = fma(t1[i], x[8 * c + i].x, acc[8 * c + i]);
-                s = fma(t2[i], x[8 * c + i].y, s);
-                s = fma(-(t1[i] * rj), t1[i], s);
-                t0[i] = -s;
-            }
-            sc_st8(sc, 3, c, t0);
-        }
-        // T4: (d_r u_theta, d_theta u_theta)
-        load_pair768<false, true, true>(x, LINE_C(1), LINE_A(1), M, tau, taud, kth0);
-        s2p<+1>(x, buf, tw, tau);
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            sc_ld8(sc, 0, c, t0);
-            sc_ld8(sc, 1, c, t1);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) acc[8 * c + i] = fma(t1[i], x[8 * c + i].y, t0[i] * x[8 * c + i].x);
-        }
-        // T5: (d_z u_theta, d_r u_z);  N_theta = -(u.grad u_theta + u_r u_theta / r);
-        //     slot 3: N_r out, U_r d_r u_z in;  x <- (N_r, N_theta)
-        load_pair768<false, false, true>(x, LINE_B(1), LINE_C(2), M, tau, taud, kth0);
-        s2p<+1>(x, buf, tw, tau);
-        sc_fence(sc);
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            double t3[8];
-            sc_ld8(sc, 0, c, t0);
-            sc_ld8(sc, 1, c, t1);
-            sc_ld8(sc, 2, c, t2);
-            sc_ld8(sc, 3, c, t3);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                double s = fma(t2[i], x[8 * c + i].x, acc[8 * c + i]);
-                s = fma(t0[i], t1[i], s);
-                t2[i] = t0[i] * x[8 * c + i].y;
-                x[8 * c + i] = mk(t3[i], -s);
-            }
-            sc_st8(sc, 3, c, t2);
-        }
-        p2s<-1>(x, buf, tw, tau);
-        store_pair768<true>(x, LINE_O(0), LINE_O(1), M, tau);
-        // T6: (d_theta u_z, d_z u_z);  N_z = -(u.grad u_z)   (buoyancy is added in k_zfwd)
-        load_pair768<true, false, true>(x, LINE_A(2), LINE_B(2), M, tau, taud, kth0);
-        s2p<+1>(x, buf, tw, tau);
-        sc_fence(sc);
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            sc_ld8(sc, 1, c, t1);
-            sc_ld8(sc, 2, c, t2);
-            sc_ld8(sc, 3, c, t0);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                double s = fma(t1[i], x[8 * c + i].x, t0[i]);
-                s = fma(t2[i], x[8 * c + i].y, s);
-                x[8 * c + i] = mk(-s, 0.0);
+            if (t >= 4) {                                      // N5: forward transform, truncation m <= M
+                p2s<-1>(x, buf, tw, tau);
+                cd* O = a.tbuf + (size_t)(t == 4 ? 0 : 2) * qstride + loff;
+                store_pair768_rt(x, O, O + qstride, t == 4, M, tau);
             }
         }
-        p2s<-1>(x, buf, tw, tau);
-        store_pair768<false>(x, LINE_O(2), nullptr, M, tau);
     }
-#undef LINE_A
-#undef LINE_B
-#undef LINE_C
-#undef LINE_O
     if constexpr (TMEM) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
