@@ -91,13 +91,27 @@ __device__ __forceinline__ ZBin z_bin(int i, int K) {
 
 constexpr int Z2_WARPS = 4;
 constexpr int Z2_THREADS = Z2_WARPS * 32;
-constexpr size_t Z2_SMEM_INV = sizeof(cd) * (size_t)(f768::XBUF * (1 + Z2_WARPS));
+constexpr size_t Z2_SMEM_X = sizeof(cd) * (size_t)(f768::XBUF * (1 + Z2_WARPS));
 constexpr size_t Z2_TILE = (size_t)f768::N * Z2_WARPS;                 // complex elements of one tile
-constexpr size_t Z2_SMEM_FWD = Z2_SMEM_INV + sizeof(cd) * Z2_TILE;     // + the second tile buffer
+constexpr size_t Z2_SMEM_FWD = Z2_SMEM_X + sizeof(cd) * Z2_TILE;     // + the second tile buffer
 
 // ------------------------------------------------------------------------------------------ k_zinv2
 // work item = (field, level, tile of 4 adjacent m); three inverse transforms per line:
-// q = 1 (i kappa f), q = 0 (f), q = 2 (D1 f).
+// q = 1 (i kappa f), q = 0 (f), q = 2 (D1 f).  Each warp stages its spectral line in a private
+// shared-memory buffer filled by cp.async one transform ahead (f for two transforms, then D1 f,
+// then the next item's f), so no line waits in registers; the three transforms share one copy of
+// the code (instruction cache).
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit_wait_all() {
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
+constexpr int Z2_LINE = 520;      // complex elements of a staged spectral line (>= 2 K + 1 = 513)
+constexpr size_t Z2_SMEM_INV = sizeof(cd) * (size_t)(f768::XBUF * (1 + Z2_WARPS) + Z2_LINE * Z2_WARPS);
+
 __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
     using namespace f768;
     const NlArgs& a = A.b;
@@ -106,43 +120,70 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
     cd* tile = tw + XBUF;                               // [768][4] tile, overlays the 4 matrices
     const int warp = threadIdx.x >> 5, tau = threadIdx.x & 31;
     cd* buf = tile + warp * XBUF;
+    cd* line = tw + XBUF * (1 + Z2_WARPS) + warp * Z2_LINE;
     load_twiddles(tw, A.tw768);
-    __syncthreads();
-    const int a23 = tau < NA ? tau : NA - 1;
     const int mtiles = a.MP / 4;
     const size_t plane = (size_t)a.M1 * a.NK;
     const size_t qstride = (size_t)a.JC * N * a.MP;
     const double taud = (double)tau;
+    const int NKc = a.NK;
 
-    int item = blockIdx.x;
-    cd F[17];
-    // loads the 17 potentially non-zero S-layout slots of one spectral line
-    auto load_line = [&](const cd* base, int it, cd* dst) {
+    // requests this warp's spectral line of item `it` from `base` (a field or its radial derivative)
+    auto fetch = [&](const cd* base, int it) {
         const int mt = it % mtiles, r = it / mtiles;
-        const int jl = r % a.nj, fi = r / a.nj;
+        const int jl = r % a.nj;
         const int m = mt * 4 + warp;
-        const bool vm = (it < A.nitems) && (m < a.M1);
-        const cd* src = base + (size_t)(a.j0 + jl) * plane + (size_t)(vm ? m : 0) * a.NK;
-        (void)fi;
-        int s = 0;
-#define NSC_LD(T)                                                  \
-    {                                                              \
-        ZBin zb = z_bin(tau + 32 * T, a.K);                        \
-        dst[s] = (vm && zb.ok) ? src[zb.kk] : mk(0.0, 0.0);        \
-        ++s;                                                       \
-    }
-        NSC_S_SLOTS(NSC_LD)
-#undef NSC_LD
+        if (m < a.M1) {
+            const cd* src = base + (size_t)(a.j0 + jl) * plane + (size_t)m * NKc;
+            for (int i = tau; i < NKc; i += 32) cp_async16(line + i, src + i);
+        }
     };
     auto field_of = [&](int it) { return (it / mtiles) / a.nj; };
-    if (item < A.nitems) load_line(a.f[field_of(item)], item, F);
+    int item = blockIdx.x;
+    if (item < A.nitems) fetch(a.f[field_of(item)], item);
+    __syncthreads();                                    // twiddles
 
     for (; item < A.nitems; item += gridDim.x) {
         const int mt = item % mtiles, r = item / mtiles;
         const int jl = r % a.nj, fi = r / a.nj;
-        cd x[32];
-        // stores the P-layout result of this warp's line into the tile and writes the tile out
-        auto emit = [&](int q) {
+        const bool vm = (mt * 4 + warp) < a.M1;
+#pragma unroll 1
+        for (int s = 0; s < 3; ++s) {
+            const int q = (s == 0) ? 1 : (s == 1 ? 0 : 2);
+            cd x[32];
+            if (s != 1) {
+                cp_async_commit_wait_all();
+                __syncwarp();
+            }
+            const double mult = (s == 0) ? A.alpha : 0.0;
+            {
+#define NSC_SET(T)                                                                              \
+    {                                                                                           \
+        const int kk = (T <= 8) ? tau + 32 * T + a.K : tau + 32 * T - N + a.K;                  \
+        const bool ok = vm && ((T <= 8) ? (tau + 32 * T <= a.K) : (tau + 32 * T >= N - a.K));   \
+        cd v = ok ? line[kk] : mk(0.0, 0.0);                                                    \
+        if (s == 0) {                                                                           \
+            const double kd = (T <= 8) ? taud + (double)(32 * T) : taud + (double)(32 * T - N); \
+            v = (mult * kd) * mul_i(v);                                                         \
+        }                                                                                       \
+        x[T] = v;                                                                               \
+    }
+                NSC_S_SLOTS(NSC_SET)
+#undef NSC_SET
+#pragma unroll
+                for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
+            }
+            if (s >= 1) {                               // the staged line is consumed: request the next one
+                __syncwarp();
+                if (s == 1) {
+                    fetch(A.dr[fi], item);
+                } else {
+                    const int nxt = item + gridDim.x;
+                    if (nxt < A.nitems) fetch(a.f[field_of(nxt)], nxt);
+                }
+            }
+            s2p<+1>(x, buf, tw, tau);
+            // P-layout result of this warp's line -> tile -> [z][m] work array in 64-byte segments
             __syncthreads();                            // all warps left their exchange matrices
             if (tau < NA) {
 #pragma unroll
@@ -157,71 +198,14 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
                 dst[(size_t)z * a.MP + (c ^ ((z >> 1) & 3))] = tile[id];
             }
             __syncthreads();                            // tile free again
-        };
-        // ---- q = 1: i kappa f
-        {
-            int s = 0;
-#define NSC_SET(T)                                                       \
-    {                                                                    \
-        const double kd = (T <= 8) ? taud + (double)(32 * T) : taud + (double)(32 * T - N); \
-        x[T] = (A.alpha * kd) * mul_i(F[s]);                             \
-        ++s;                                                             \
-    }
-            NSC_S_SLOTS(NSC_SET)
-#undef NSC_SET
-#pragma unroll
-            for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
         }
-        s2p<+1>(x, buf, tw, tau);
-        emit(1);
-        // ---- q = 0: f  (F dies here); the D1 f line is requested before the transform
-        {
-            int s = 0;
-#define NSC_SET(T) \
-    {              \
-        x[T] = F[s]; \
-        ++s;       \
     }
-            NSC_S_SLOTS(NSC_SET)
-#undef NSC_SET
-#pragma unroll
-            for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
-        }
-        cd D[17];
-        load_line(A.dr[fi], item, D);
-        s2p<+1>(x, buf, tw, tau);
-        emit(0);
-        // ---- q = 2: D1 f; the next item's f line is requested before the transform
-        {
-            int s = 0;
-#define NSC_SET(T) \
-    {              \
-        x[T] = D[s]; \
-        ++s;       \
-    }
-            NSC_S_SLOTS(NSC_SET)
-#undef NSC_SET
-#pragma unroll
-            for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
-        }
-        const int nxt = item + gridDim.x;
-        if (nxt < A.nitems) load_line(a.f[field_of(nxt)], nxt, F);
-        s2p<+1>(x, buf, tw, tau);
-        emit(2);
-    }
-    (void)a23;
+    cp_async_commit_wait_all();
 }
 
 // ------------------------------------------------------------------------------------------ k_zfwd2
 // work item = (field, level, tile of 4 adjacent m).  The [768][4] tile of theta-transformed
 // products arrives by cp.async (64-byte segments) while the previous item is being transformed.
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
-    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit_wait_all() {
-    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
-}
 
 __global__ void __launch_bounds__(Z2_THREADS, 2) k_zfwd2(Nl2Args A) {
     using namespace f768;
