@@ -138,6 +138,7 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
         c->t768 = (c->Nt == 768 && c->M <= 256 && c->nf == 3) ? ((variant >> 1) & 3) : 0;
         if (c->t768 > 2) c->t768 = 2;
     }
+    if (const char* ev = getenv("NSC_LIN_VARIANT")) c->lin_fused = atoi(ev) != 0;
     int rc = build_plan(c);
     if (!rc && c->z768)
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->DR[i], c->F, false);
@@ -148,6 +149,7 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->N0[i], c->F, false);
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->N1[i], c->F, false);
         if (!rc) rc = dev_alloc(c, &c->G, c->F, false);
+        if (!rc && c->lin_fused) rc = dev_alloc(c, &c->DP, c->F, true);
         if (!rc) rc = dev_alloc(c, &c->zbuf, (size_t)3 * c->nf * c->JC * c->Nz * c->MP, true);
         if (!rc) rc = dev_alloc(c, &c->tbuf, (size_t)c->nf * c->JC * c->Nz * c->MP, true);
     }
@@ -227,11 +229,21 @@ static int copy_state(nsc_ctx* c, const void* const* src, void* const* dst, cuda
     return NSC_OK;
 }
 
+// derived arrays of a new state: D1 p for the fused linear path
+static int after_set_state(nsc_ctx* c) {
+    if (c->DP) {
+        int rc = launch_radial_derivative(c, c->state[4], c->DP);
+        if (rc) return rc;
+    }
+    c->have_state = true;
+    return NSC_OK;
+}
+
 int nsc_set_state(nsc_ctx* c, const void* ur, const void* uth, const void* uz, const void* T, const void* p) {
     if (!c) return NSC_EINVAL;
     const void* src[5] = {ur, uth, uz, T, p};
     int rc = copy_state(c, src, nullptr, cudaMemcpyDeviceToDevice, true);
-    if (!rc) c->have_state = true;
+    if (!rc) rc = after_set_state(c);
     return rc;
 }
 
@@ -248,8 +260,7 @@ int nsc_set_state_host(nsc_ctx* c, const void* ur, const void* uth, const void* 
     int rc = copy_state(c, src, nullptr, cudaMemcpyHostToDevice, true);
     if (rc) return rc;
     NSC_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->have_state = true;
-    return NSC_OK;
+    return after_set_state(c);
 }
 
 int nsc_get_state_host(nsc_ctx* c, void* ur, void* uth, void* uz, void* T, void* p) {

@@ -10,6 +10,7 @@
 // and are the same for +k and -k, so one thread serves the pair (m, |k|).  They are LU-factored
 // without pivoting inside their row envelope (no fill-in outside it) once per dt (Helmholtz) /
 // once per context (Poisson); the solves stream the factors with pair-major (coalesced) access.
+#include <cstdint>
 #include "nsc_internal.h"
 
 namespace nsc {
@@ -196,6 +197,7 @@ struct LinArgs {
     cd* G;                 // divergence / phi
     cd* dst[MAXF];         // corrected fields
     cd* p_dst;             // new pressure (may be null)
+    cd* DP;                // D1 p, updated with D1 phi / dt when p_dst is set (may be null)
     const double *D1, *L0, *rinv, *nm, *kap;
     const int* s0;
     int N_r, M1, NK, K, nf;
@@ -331,7 +333,335 @@ __global__ void __launch_bounds__(128) k_correct(LinArgs a) {
     a.dst[1][o] = a.W[1][o] - (a.nm[m] * ri) * mul_i(phi);
     a.dst[2][o] = a.W[2][o] - a.kap[kk] * mul_i(phi);
     if (a.nf == 4 && a.dst[3] != a.W[3]) a.dst[3][o] = a.W[3][o];
-    if (a.p_dst) a.p_dst[o] = a.p[o] + (1.0 / a.dt) * phi;
+    if (a.p_dst) {
+        a.p_dst[o] = a.p[o] + (1.0 / a.dt) * phi;
+        if (a.DP) a.DP[o] = a.DP[o] + (1.0 / a.dt) * gphi;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Fused sweeps (default path).  One thread serves one (mode, field): field 0 u_+, 1 u_-, 2 u_z, 3 T;
+// the factors of the pair (m, |k|) are read by both of its modes (the second read hits L2).
+//
+// With A = I - c dt nu L and gamma = (1 - c) / c the right-hand side of step L1 is
+//     u + dt (1 - c) nu L u + dt R  =  u / c - gamma A u + dt R        (R = E - pressure-gradient term),
+// so   x = A^-1 (u / c + dt R) - gamma u   at interior rows: no radial stencil acts on u.  D1 p is kept
+// as an array of its own (DP), updated by k_correct with D1 phi / dt (D1 is linear).  Wall rows of A are identity rows: b_wall = BC + gamma u_wall.
+//
+//   k_rhs_fwd  (marching up)   : b from u, E, p, D1 p, forward
+//                                substitution with the stored L factors, y -> W[field]
+//   k_bwd_div  (marching down) : back substitution, - gamma u, recombination of u_+- into
+//                                (u_r*, u_theta*), divergence g (L2, L3) -- see below
+struct FusedArgs {
+    const cd* u[MAXF];
+    const cd* p;
+    const cd* DP;          // D1 p (interior rows)
+    const cd* E0[MAXF];
+    const cd* E1[MAXF];    // may be null
+    cd* W[MAXF];
+    cd* G;
+    const double* L[MAXF];
+    const double* U[MAXF];
+    const int *lo, *hi, *offL, *offU;
+    const double *D1, *rinv, *nm, *kap;
+    const int* s0;
+    int N_r, M1, NK, K, P, nf;
+    int offL4, offU4;      // offL[4], offU[4]: the interior rows 4 .. N_r - 5 have regular offsets
+    double dt, c, w0, w1, Re_i, Re_o;
+};
+
+constexpr int FW = 8;       // forward / backward substitution window (rows), Helmholtz envelope <= 7
+constexpr int FWI = 4;      // interior lower / upper width
+
+__device__ __forceinline__ cd ldcs(const cd* p) {
+    const double2 v = __ldcs(reinterpret_cast<const double2*>(p));
+    return mk(v.x, v.y);
+}
+
+// ---- row pipeline: every row's operands arrive in shared memory by cp.async, PIPE - 1 rows ahead of
+// the row being eliminated, so that the marching threads never wait on HBM with a single row in flight
+constexpr int PBK = 64;     // modes per block
+constexpr int PIPE = 4;     // shared-memory row slots
+__device__ __forceinline__ void cpa16(void* s, const void* g) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(s)), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cpa8(void* s, const void* g) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(s)), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cpa_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPEND> __device__ __forceinline__ void cpa_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(NPEND) : "memory");
+}
+
+// k_rhs_fwd: block = (PBK modes) x (NF fields).  Slot arrays: u[NF], p, DP, E0[NF], E1[NF] (if present).
+template <int NF> struct FwdSlot {
+    cd fld[3 * NF + 2][PBK];
+    double L[NF][FWI][PBK];
+};
+
+template <int NF>
+__global__ void __launch_bounds__(PBK * NF) k_rhs_fwd(FusedArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    FwdSlot<NF>* slots = reinterpret_cast<FwdSlot<NF>*>(smem_raw);
+    const int tx = threadIdx.x, fld = threadIdx.y;
+    const int plane_i = a.M1 * a.NK;
+    const int e0 = blockIdx.x * PBK + tx;
+    const bool valid = e0 < plane_i;
+    const int e = valid ? e0 : plane_i - 1;
+    const int m = e / a.NK, kk = e % a.NK;
+    const int ka = kk >= a.K ? kk - a.K : a.K - kk;
+    const size_t P = a.P;
+    const size_t plane = (size_t)plane_i;
+    const int N = a.N_r;
+    const double n = a.nm[m], kap = a.kap[kk];
+    const double ic = 1.0 / a.c, gam = (1.0 - a.c) / a.c, dt = a.dt;
+    const bool m00 = (m == 0 && ka == 0);
+    const bool two = a.E1[0] != nullptr;
+    const int narr = two ? 3 * NF + 2 : 2 * NF + 2;
+    const double* Lf = (fld == 0 ? a.L[0] : fld == 1 ? a.L[1] : fld == 2 ? a.L[2] : a.L[3]) + (size_t)m * (a.K + 1) + ka;
+    cd* Wf = fld == 0 ? a.W[0] : fld == 1 ? a.W[1] : fld == 2 ? a.W[2] : a.W[3];
+    const int ja = FWI, jb = N - FWI;                    // interior rows [ja, jb): nl = 4, offL regular
+    // array q of the slot: 0..NF-1 u, NF p, NF+1 DP, NF+2.. E0, 2NF+2.. E1
+    auto src_of = [&](int q) -> const cd* {
+        if (q < NF) return q == 0 ? a.u[0] : q == 1 ? a.u[1] : q == 2 ? a.u[2] : a.u[3];
+        if (q == NF) return a.p;
+        if (q == NF + 1) return a.DP;
+        q -= NF + 2;
+        if (q < NF) return q == 0 ? a.E0[0] : q == 1 ? a.E0[1] : q == 2 ? a.E0[2] : a.E0[3];
+        q -= NF;
+        return q == 0 ? a.E1[0] : q == 1 ? a.E1[1] : q == 2 ? a.E1[2] : a.E1[3];
+    };
+    auto issue = [&](int j) {
+        if (j < N) {
+            FwdSlot<NF>& s = slots[j % PIPE];
+            const size_t o = (size_t)j * plane + e;
+            for (int q = fld; q < narr; q += NF) cpa16(&s.fld[q][tx], src_of(q) + o);
+            if (j >= ja && j < jb) {
+                const double* Lr = Lf + (size_t)(a.offL4 + FWI * (j - ja)) * P;
+#pragma unroll
+                for (int i = 0; i < FWI; ++i) cpa8(&s.L[fld][i][tx], Lr + (size_t)i * P);
+            }
+        }
+        cpa_commit();
+    };
+    cd w[FW];                                           // w[FW-1] = most recent row
+#pragma unroll
+    for (int i = 0; i < FW; ++i) w[i] = mk(0.0, 0.0);
+#pragma unroll
+    for (int d = 0; d < PIPE - 1; ++d) issue(d);
+    for (int j = 0; j < N; ++j) {
+        cpa_wait<PIPE - 2>();
+        __syncthreads();
+        issue(j + PIPE - 1);
+        const FwdSlot<NF>& s = slots[j % PIPE];
+        const bool wall = (j == 0 || j == N - 1);
+        cd b;
+        if (fld < 2) {
+            const double sg = fld == 0 ? 1.0 : -1.0;
+            const cd ur = s.fld[0][tx], ut = s.fld[1][tx];
+            const cd u = mk(ur.x - sg * ut.y, ur.y + sg * ut.x);         // u_r + sg i u_theta
+            if (wall) {
+                const double v = m00 ? sg * (j == 0 ? a.Re_i : a.Re_o) : 0.0;
+                b = mk(gam * u.x, v + gam * u.y);
+            } else {
+                cd Er = a.w0 * s.fld[NF + 2][tx], Et = a.w0 * s.fld[NF + 3][tx];
+                if (two) {
+                    Er = Er + a.w1 * s.fld[2 * NF + 2][tx];
+                    Et = Et + a.w1 * s.fld[2 * NF + 3][tx];
+                }
+                const cd Dp = s.fld[NF + 1][tx], pr = s.fld[NF][tx];
+                const double nr = sg * n * a.rinv[j];
+                // R = (E_r + sg i E_theta) - (D1 p - sg (n / r) p)
+                const cd R = mk(Er.x - sg * Et.y - Dp.x + nr * pr.x, Er.y + sg * Et.x - Dp.y + nr * pr.y);
+                b = mk(fma(dt, R.x, ic * u.x), fma(dt, R.y, ic * u.y));
+            }
+        } else {
+            const cd u = s.fld[fld][tx];
+            if (wall) {
+                const double v = (fld == 3 && m00) ? (j == 0 ? 0.5 : -0.5) : 0.0;
+                b = mk(v + gam * u.x, gam * u.y);
+            } else {
+                cd E = a.w0 * s.fld[NF + 2 + fld][tx];
+                if (two) E = E + a.w1 * s.fld[2 * NF + 2 + fld][tx];
+                if (fld == 2) {                         // - i kappa p
+                    const cd pr = s.fld[NF][tx];
+                    E = mk(E.x + kap * pr.y, E.y - kap * pr.x);
+                }
+                b = mk(fma(dt, E.x, ic * u.x), fma(dt, E.y, ic * u.y));
+            }
+        }
+        // forward substitution: y_j = b_j - sum_i L[j][i] y_{lo + i}
+        if (j >= ja && j < jb) {
+#pragma unroll
+            for (int i = 0; i < FWI; ++i) {
+                const double l = s.L[fld][i][tx];
+                b.x = fma(-l, w[FW - FWI + i].x, b.x);
+                b.y = fma(-l, w[FW - FWI + i].y, b.y);
+            }
+        } else {
+            const int nl = j - a.lo[j];
+            const double* Lr = Lf + (size_t)a.offL[j] * P;
+#pragma unroll
+            for (int q = 0; q < FW; ++q) {
+                const int i = q - (FW - nl);
+                if (i >= 0) {
+                    const double l = Lr[(size_t)i * P];
+                    b.x = fma(-l, w[q].x, b.x);
+                    b.y = fma(-l, w[q].y, b.y);
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < FW - 1; ++q) w[q] = w[q + 1];
+        w[FW - 1] = b;
+        if (valid) Wf[(size_t)j * plane + e] = b;
+    }
+    cpa_wait<0>();
+}
+
+// k_bwd_div: block = (PBK modes) x (NF field roles + 1 divergence role), marching down.  Field role f
+// back-substitutes its system, subtracts gamma u_f and hands x_f(j) to the divergence role through
+// a double-buffered shared-memory slot (one barrier per row, the divergence role runs one row behind); the divergence role forms
+// u_r* = (x_+ + x_-)/2, u_theta* = (x_+ - x_-)/(2i), stores them and emits
+// g = D1 u_r* + u_r*/r + (i n / r) u_theta* + i kappa u_z* four rows behind the march, from a ring of the
+// last rows of u_r* in shared memory (g = 0 in the wall rows).  Slot arrays: y[NF] (in W), u[NF], U rows.
+template <int NF> struct BwdSlot {
+    cd fld[2 * NF][PBK];
+    double U[NF][FWI + 1][PBK];
+};
+
+template <int NF>
+__global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    BwdSlot<NF>* slots = reinterpret_cast<BwdSlot<NF>*>(smem_raw);
+    __shared__ cd exch[2][3][PBK];
+    __shared__ cd ring_ur[16][PBK];                     // u_r* of the last rows (column tx is private to the
+    __shared__ cd ring_g[FW][PBK];                      // divergence-role thread tx), stencil-free part of g
+    const int tx = threadIdx.x, role = threadIdx.y;
+    const int plane_i = a.M1 * a.NK;
+    const int e0 = blockIdx.x * PBK + tx;
+    const bool valid = e0 < plane_i;
+    const int e = valid ? e0 : plane_i - 1;
+    const int m = e / a.NK, kk = e % a.NK;
+    const int ka = kk >= a.K ? kk - a.K : a.K - kk;
+    const size_t P = a.P;
+    const size_t plane = (size_t)plane_i;
+    const int N = a.N_r;
+    const double n = a.nm[m], kap = a.kap[kk];
+    const double gam = (1.0 - a.c) / a.c;
+    const bool is_field = role < NF;
+    const int f = is_field ? role : 0;
+    const double* Uf = (f == 0 ? a.U[0] : f == 1 ? a.U[1] : f == 2 ? a.U[2] : a.U[3]) + (size_t)m * (a.K + 1) + ka;
+    cd* Wf = f == 0 ? a.W[0] : f == 1 ? a.W[1] : f == 2 ? a.W[2] : a.W[3];
+    const double sg = f == 0 ? 1.0 : -1.0;
+    const int ja = FWI, jb = N - FWI;                    // interior rows [ja, jb): nu = 4, offU regular
+    auto src_of = [&](int q) -> const cd* {
+        if (q < NF) return q == 0 ? a.W[0] : q == 1 ? a.W[1] : q == 2 ? a.W[2] : a.W[3];
+        q -= NF;
+        return q == 0 ? a.u[0] : q == 1 ? a.u[1] : q == 2 ? a.u[2] : a.u[3];
+    };
+    // row j travels in slot (N - 1 - j) % PIPE
+    auto issue = [&](int j) {
+        if (j >= 0) {
+            BwdSlot<NF>& s = slots[(N - 1 - j) % PIPE];
+            const size_t o = (size_t)j * plane + e;
+            for (int q = role; q < 2 * NF; q += NF + 1) cpa16(&s.fld[q][tx], src_of(q) + o);
+            if (is_field && j >= ja && j < jb) {
+                const double* Ur = Uf + (size_t)(a.offU4 + (FWI + 1) * (j - ja)) * P;
+#pragma unroll
+                for (int i = 0; i <= FWI; ++i) cpa8(&s.U[f][i][tx], Ur + (size_t)i * P);
+            }
+        }
+        cpa_commit();
+    };
+    cd w[FW];                                           // back-substitution window, w[0] = x_{j+1}
+#pragma unroll
+    for (int i = 0; i < FW; ++i) w[i] = mk(0.0, 0.0);
+    // divergence role, row j (its x_+, x_-, x_z were left in exch[j & 1] one iteration earlier)
+    auto div_row = [&](int j) {
+        const size_t o = (size_t)j * plane + e;
+        const cd xa = exch[j & 1][0][tx], xb = exch[j & 1][1][tx], xz = exch[j & 1][2][tx];
+        const cd ur = 0.5 * (xa + xb);
+        const cd ut = 0.5 * mul_mi(xa - xb);
+        if (valid) {
+            a.W[0][o] = ur;
+            a.W[1][o] = ut;
+        }
+        const double ri = a.rinv[j], nr = n * ri;
+        ring_ur[j & 15][tx] = ur;
+        // u_r*/r + (i n / r) u_theta* + i kappa u_z*
+        ring_g[j & (FW - 1)][tx] = mk(ri * ur.x - nr * ut.y - kap * xz.y, ri * ur.y + nr * ut.x + kap * xz.x);
+        if (valid) {
+            if (j == N - 1 || j == 0) a.G[o] = mk(0.0, 0.0);
+            if (j <= N - NPT) {
+                // rows whose stencil is the window j .. j + 8
+                const int c_lo = (j == 0) ? 1 : j + NPT / 2;
+                const int c_hi = (j == N - NPT) ? N - 2 : j + NPT / 2;
+                for (int jc = c_lo; jc <= c_hi; ++jc) {
+                    const double* d = a.D1 + jc * NPT;
+                    cd g = ring_g[jc & (FW - 1)][tx];
+#pragma unroll
+                    for (int l = 0; l < NPT; ++l) {
+                        const double wt = __ldg(d + l);
+                        const cd v = ring_ur[(j + l) & 15][tx];
+                        g.x = fma(wt, v.x, g.x);
+                        g.y = fma(wt, v.y, g.y);
+                    }
+                    a.G[(size_t)jc * plane + e] = g;
+                }
+            }
+        }
+    };
+#pragma unroll
+    for (int d = 0; d < PIPE - 1; ++d) issue(N - 1 - d);
+    for (int j = N - 1; j >= 0; --j) {
+        cpa_wait<PIPE - 2>();
+        __syncthreads();                                 // row j has arrived; exch[(j + 1) & 1] is complete
+        issue(j - (PIPE - 1));
+        const BwdSlot<NF>& s = slots[(N - 1 - j) % PIPE];
+        const size_t o = (size_t)j * plane + e;
+        if (is_field) {
+            cd y = s.fld[f][tx];
+            if (j >= ja && j < jb) {
+#pragma unroll
+                for (int q = 0; q < FWI; ++q) {
+                    const double u = s.U[f][q + 1][tx];
+                    y.x = fma(-u, w[q].x, y.x);
+                    y.y = fma(-u, w[q].y, y.y);
+                }
+                y = s.U[f][0][tx] * y;
+            } else {
+                const int nu = a.hi[j] - j;
+                const double* Ur = Uf + (size_t)a.offU[j] * P;
+#pragma unroll
+                for (int q = 0; q < FW; ++q) {
+                    if (q < nu) {
+                        const double u = Ur[(size_t)(q + 1) * P];
+                        y.x = fma(-u, w[q].x, y.x);
+                        y.y = fma(-u, w[q].y, y.y);
+                    }
+                }
+                y = Ur[0] * y;
+            }
+#pragma unroll
+            for (int q = FW - 1; q > 0; --q) w[q] = w[q - 1];
+            w[0] = y;
+            cd u;                                        // u_f of the state the sub-step starts from
+            if (f < 2) {
+                const cd ur = s.fld[NF][tx], ut = s.fld[NF + 1][tx];
+                u = mk(ur.x - sg * ut.y, ur.y + sg * ut.x);
+            } else {
+                u = s.fld[NF + f][tx];
+            }
+            const cd x = mk(fma(-gam, u.x, y.x), fma(-gam, u.y, y.y));
+            if (f < 3) exch[j & 1][f][tx] = x;
+            if (f >= 2 && valid) Wf[o] = x;
+        }
+        if (!is_field && j < N - 1) div_row(j + 1);      // one row behind the field roles
+    }
+    __syncthreads();
+    if (!is_field) div_row(0);
+    cpa_wait<0>();
 }
 
 // ------------------------------------------------------------------------------------------
@@ -448,6 +778,7 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
     a.p = c->state[4];
     a.G = c->G;
     a.p_dst = p_dst;
+    a.DP = c->lin_fused ? c->DP : nullptr;
     a.D1 = c->t.D1;
     a.L0 = c->t.L0;
     a.rinv = c->t.rinv;
@@ -468,6 +799,73 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
     a.Re_o = c->p.Re_o;
     const int plane = c->M1 * c->NK;
     dim3 gridp((plane + 127) / 128, c->N_r);
+    if (c->lin_fused) {
+        FusedArgs fa{};
+        for (int i = 0; i < c->nf; ++i) {
+            fa.u[i] = c->state[i];
+            fa.E0[i] = E0[i];
+            fa.E1[i] = E1 ? E1[i] : nullptr;
+            fa.W[i] = c->W[i];
+            const BandFactors& bf = (i == 3 && c->facT_shared) ? c->facH[2] : c->facH[i];
+            fa.L[i] = bf.L;
+            fa.U[i] = bf.U;
+        }
+        fa.p = c->state[4];
+        fa.G = c->G;
+        fa.lo = c->shH.lo;
+        fa.hi = c->shH.hi;
+        fa.offL = c->shH.offL;
+        fa.offU = c->shH.offU;
+        fa.D1 = c->t.D1;
+        fa.rinv = c->t.rinv;
+        fa.nm = c->t.nm;
+        fa.kap = c->t.kap;
+        fa.s0 = c->t.s0;
+        fa.N_r = c->N_r;
+        fa.M1 = c->M1;
+        fa.NK = c->NK;
+        fa.K = c->K;
+        fa.P = c->P;
+        fa.nf = c->nf;
+        fa.dt = dt;
+        fa.c = c->p.c;
+        fa.w0 = w0;
+        fa.w1 = w1;
+        fa.Re_i = c->p.Re_i;
+        fa.Re_o = c->p.Re_o;
+        const int nb = (plane + PBK - 1) / PBK;
+        fa.DP = c->DP;
+        fa.offL4 = c->shH.h_offL[FWI];
+        fa.offU4 = c->shH.h_offU[FWI];
+        static bool attr_done = false;
+        if (!attr_done) {
+            cudaFuncSetAttribute(k_rhs_fwd<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE * sizeof(FwdSlot<3>)));
+            cudaFuncSetAttribute(k_rhs_fwd<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE * sizeof(FwdSlot<4>)));
+            cudaFuncSetAttribute(k_bwd_div<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE * sizeof(BwdSlot<3>)));
+            cudaFuncSetAttribute(k_bwd_div<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE * sizeof(BwdSlot<4>)));
+            attr_done = true;
+        }
+        prof_begin(c, NSC_K_RHS);
+        if (c->nf == 3)
+            k_rhs_fwd<3><<<nb, dim3(PBK, 3), PIPE * sizeof(FwdSlot<3>), c->stream>>>(fa);
+        else
+            k_rhs_fwd<4><<<nb, dim3(PBK, 4), PIPE * sizeof(FwdSlot<4>), c->stream>>>(fa);
+        prof_end(c);
+        NSC_CUDA(c, cudaGetLastError());
+        prof_begin(c, NSC_K_HELMHOLTZ);
+        if (c->nf == 3)
+            k_bwd_div<3><<<nb, dim3(PBK, 4), PIPE * sizeof(BwdSlot<3>), c->stream>>>(fa);
+        else
+            k_bwd_div<4><<<nb, dim3(PBK, 5), PIPE * sizeof(BwdSlot<4>), c->stream>>>(fa);
+        prof_end(c);
+        NSC_CUDA(c, cudaGetLastError());
+        if ((rc = run_solve(c, c->facP, c->shP, c->G, true))) return rc;
+        prof_begin(c, NSC_K_CORRECT);
+        k_correct<<<gridp, 128, 0, c->stream>>>(a);
+        prof_end(c);
+        NSC_CUDA(c, cudaGetLastError());
+        return NSC_OK;
+    }
     prof_begin(c, NSC_K_RHS);
     k_rhs<<<gridp, 128, 0, c->stream>>>(a);
     prof_end(c);

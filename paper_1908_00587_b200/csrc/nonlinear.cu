@@ -22,6 +22,19 @@ static const LenEntry* find_len(int n) {
 
 bool fft_length_supported(int n) { return find_len(n) != nullptr; }
 
+int launch_radial_derivative(nsc_ctx* c, const cd* f, cd* out) {
+    DrArgs d{};
+    d.f[0] = f;
+    d.out[0] = out;
+    d.D1 = c->t.D1;
+    d.N_r = c->N_r;
+    d.plane = (size_t)c->M1 * c->NK;
+    prof_begin(c, NSC_K_DR);
+    if (int e = launch_dr(d, 1, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_dr launch");
+    prof_end(c);
+    return NSC_OK;
+}
+
 int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
     const LenEntry* lz = find_len(c->Nz);
     const LenEntry* lt = find_len(c->Nt);

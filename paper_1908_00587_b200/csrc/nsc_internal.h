@@ -60,6 +60,7 @@ struct nsc_ctx {
     nsc::cd* state[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // u_r, u_theta, u_z, T, p
     nsc::cd* W[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};        // sub-step work / predictor state
     nsc::cd* G = nullptr;                 // divergence / phi
+    nsc::cd* DP = nullptr;                // D1 p of the state (fused linear path)
     nsc::cd* N0[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* N1[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* zbuf = nullptr;              // [3 nf][JC][N_z][MP]  z-transformed f, dz f, dr f
@@ -73,6 +74,7 @@ struct nsc_ctx {
     bool facT_shared = false;             // T shares the u_z factors (Pr == 1)
     double fac_dt = 0.0;                  // dt the Helmholtz factors were built for (0: none)
     bool facP_ready = false;
+    bool lin_fused = true;                // fused sweeps k_rhs_fwd / k_bwd_div (NSC_LIN_VARIANT=0: separate kernels)
     bool have_state = false;
     std::string err;
     long long launches = 0;
@@ -92,6 +94,8 @@ int build_plan(nsc_ctx* c);
 
 // nonlinear.cu : N(f[0..nf-1]) -> out[0..nf-1]   (steps N1-N6)
 int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out);
+// out = D1 f (radial derivative of one spectral field, all rows)
+int launch_radial_derivative(nsc_ctx* c, const cd* f, cd* out);
 
 // linear.cu
 int ensure_factors(nsc_ctx* c, double dt);
