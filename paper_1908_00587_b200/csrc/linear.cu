@@ -380,8 +380,24 @@ __device__ __forceinline__ cd ldcs(const cd* p) {
 
 // ---- row pipeline: every row's operands arrive in shared memory by cp.async, PIPE - 1 rows ahead of
 // the row being eliminated, so that the marching threads never wait on HBM with a single row in flight
-constexpr int PBK = 64;     // modes per block
-constexpr int PIPE = 4;     // shared-memory row slots
+#ifndef NSC_PBK
+#define NSC_PBK 64
+#endif
+constexpr int PBK = NSC_PBK;     // modes per block
+// shared-memory row slots of the four sweeps (rows in flight = slots - 1)
+#ifndef NSC_PIPE_F
+#define NSC_PIPE_F 3
+#endif
+#ifndef NSC_PIPE_B
+#define NSC_PIPE_B 3
+#endif
+#ifndef NSC_PIPE_PF
+#define NSC_PIPE_PF 3
+#endif
+#ifndef NSC_PIPE_PB
+#define NSC_PIPE_PB 3
+#endif
+constexpr int PIPE_F = NSC_PIPE_F, PIPE_B = NSC_PIPE_B, PIPE_PF = NSC_PIPE_PF, PIPE_PB = NSC_PIPE_PB;
 __device__ __forceinline__ void cpa16(void* s, const void* g) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(s)), "l"(g) : "memory");
 }
@@ -433,7 +449,7 @@ __global__ void __launch_bounds__(PBK * NF) k_rhs_fwd(FusedArgs a) {
     };
     auto issue = [&](int j) {
         if (j < N) {
-            FwdSlot<NF>& s = slots[j % PIPE];
+            FwdSlot<NF>& s = slots[j % PIPE_F];
             const size_t o = (size_t)j * plane + e;
             for (int q = fld; q < narr; q += NF) cpa16(&s.fld[q][tx], src_of(q) + o);
             if (j >= ja && j < jb) {
@@ -448,12 +464,12 @@ __global__ void __launch_bounds__(PBK * NF) k_rhs_fwd(FusedArgs a) {
 #pragma unroll
     for (int i = 0; i < FW; ++i) w[i] = mk(0.0, 0.0);
 #pragma unroll
-    for (int d = 0; d < PIPE - 1; ++d) issue(d);
+    for (int d = 0; d < PIPE_F - 1; ++d) issue(d);
     for (int j = 0; j < N; ++j) {
-        cpa_wait<PIPE - 2>();
+        cpa_wait<PIPE_F - 2>();
         __syncthreads();
-        issue(j + PIPE - 1);
-        const FwdSlot<NF>& s = slots[j % PIPE];
+        issue(j + PIPE_F - 1);
+        const FwdSlot<NF>& s = slots[j % PIPE_F];
         const bool wall = (j == 0 || j == N - 1);
         cd b;
         if (fld < 2) {
@@ -560,10 +576,10 @@ __global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
         q -= NF;
         return q == 0 ? a.u[0] : q == 1 ? a.u[1] : q == 2 ? a.u[2] : a.u[3];
     };
-    // row j travels in slot (N - 1 - j) % PIPE
+    // row j travels in slot (N - 1 - j) % PIPE_B
     auto issue = [&](int j) {
         if (j >= 0) {
-            BwdSlot<NF>& s = slots[(N - 1 - j) % PIPE];
+            BwdSlot<NF>& s = slots[(N - 1 - j) % PIPE_B];
             const size_t o = (size_t)j * plane + e;
             for (int q = role; q < 2 * NF; q += NF + 1) cpa16(&s.fld[q][tx], src_of(q) + o);
             if (is_field && j >= ja && j < jb) {
@@ -613,12 +629,12 @@ __global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
         }
     };
 #pragma unroll
-    for (int d = 0; d < PIPE - 1; ++d) issue(N - 1 - d);
+    for (int d = 0; d < PIPE_B - 1; ++d) issue(N - 1 - d);
     for (int j = N - 1; j >= 0; --j) {
-        cpa_wait<PIPE - 2>();
+        cpa_wait<PIPE_B - 2>();
         __syncthreads();                                 // row j has arrived; exch[(j + 1) & 1] is complete
-        issue(j - (PIPE - 1));
-        const BwdSlot<NF>& s = slots[(N - 1 - j) % PIPE];
+        issue(j - (PIPE_B - 1));
+        const BwdSlot<NF>& s = slots[(N - 1 - j) % PIPE_B];
         const size_t o = (size_t)j * plane + e;
         if (is_field) {
             cd y = s.fld[f][tx];
@@ -662,6 +678,243 @@ __global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
     __syncthreads();
     if (!is_field) div_row(0);
     cpa_wait<0>();
+}
+
+// ------------------------------------------------------------------------------------------
+// Pressure stage of the fused path (L4, L5), one thread per mode, same row pipeline:
+//   k_poisson_fwd (marching up)  : forward substitution of P phi = g with the stored L factors, in place in G
+//   k_poisson_bwd_correct (down) : back substitution, phi kept in a shared-memory ring (never stored);
+//                                  four rows behind the march  u = u* - (G~ phi, (i n / r) phi, i kappa phi),
+//                                  p += phi / dt, D1 p += D1 phi / dt, u_r(0,0) := 0 (O8)
+struct PoisArgs {
+    cd* G;
+    const double* L;
+    const double* U;
+    const int *lo, *hi, *offL, *offU;
+    int jaL, jbL, offLa;   // rows [jaL, jbL): nl = PWI, offL[j] = offLa + PWI (j - jaL)
+    int jaU, jbU, offUa;   // rows [jaU, jbU): nu = PWI, offU[j] = offUa + (PWI + 1)(j - jaU)
+    const cd* W[MAXF];     // u_r*, u_theta*, u_z*, T
+    cd* dst[MAXF];
+    const cd* p;
+    cd* p_dst;             // may be null: pressure discarded
+    cd* DP;
+    const double *D1, *rinv, *nm, *kap;
+    const int* s0;
+    int N_r, M1, NK, K, P, nf;
+    int copyT;             // dst[3] != W[3]
+    double dt;
+};
+
+constexpr int PBP = 128;    // modes per block, forward sweep
+constexpr int PBB = 64;     // modes per block, backward sweep + correction
+constexpr int PW = 12;      // substitution window (Poisson envelope <= 12)
+constexpr int PWI = 8;      // interior lower / upper width
+
+struct PFwdSlot {
+    cd g[PBP];
+    double L[PWI][PBP];
+};
+
+__global__ void __launch_bounds__(PBP) k_poisson_fwd(PoisArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PFwdSlot* slots = reinterpret_cast<PFwdSlot*>(smem_raw);
+    const int tx = threadIdx.x;
+    const int plane_i = a.M1 * a.NK;
+    const int e0 = blockIdx.x * PBP + tx;
+    const bool valid = e0 < plane_i;
+    const int e = valid ? e0 : plane_i - 1;
+    const int m = e / a.NK, kk = e % a.NK;
+    const int ka = kk >= a.K ? kk - a.K : a.K - kk;
+    const size_t P = a.P;
+    const size_t plane = (size_t)plane_i;
+    const int N = a.N_r;
+    const double* Lf = a.L + (size_t)m * (a.K + 1) + ka;
+    auto issue = [&](int j) {
+        if (j < N) {
+            PFwdSlot& s = slots[j % PIPE_PF];
+            cpa16(&s.g[tx], a.G + (size_t)j * plane + e);
+            if (j >= a.jaL && j < a.jbL) {
+                const double* Lr = Lf + (size_t)(a.offLa + PWI * (j - a.jaL)) * P;
+#pragma unroll
+                for (int i = 0; i < PWI; ++i) cpa8(&s.L[i][tx], Lr + (size_t)i * P);
+            }
+        }
+        cpa_commit();
+    };
+    cd w[PW];                                           // w[PW-1] = most recent row
+#pragma unroll
+    for (int i = 0; i < PW; ++i) w[i] = mk(0.0, 0.0);
+#pragma unroll
+    for (int d = 0; d < PIPE_PF - 1; ++d) issue(d);
+    for (int j = 0; j < N; ++j) {
+        cpa_wait<PIPE_PF - 2>();
+        __syncthreads();
+        issue(j + PIPE_PF - 1);
+        const PFwdSlot& s = slots[j % PIPE_PF];
+        cd b = s.g[tx];
+        if (j >= a.jaL && j < a.jbL) {
+#pragma unroll
+            for (int i = 0; i < PWI; ++i) {
+                const double l = s.L[i][tx];
+                b.x = fma(-l, w[PW - PWI + i].x, b.x);
+                b.y = fma(-l, w[PW - PWI + i].y, b.y);
+            }
+        } else {
+            const int nl = j - a.lo[j];
+            const double* Lr = Lf + (size_t)a.offL[j] * P;
+#pragma unroll
+            for (int q = 0; q < PW; ++q) {
+                const int i = q - (PW - nl);
+                if (i >= 0) {
+                    const double l = Lr[(size_t)i * P];
+                    b.x = fma(-l, w[q].x, b.x);
+                    b.y = fma(-l, w[q].y, b.y);
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < PW - 1; ++q) w[q] = w[q + 1];
+        w[PW - 1] = b;
+        if (valid) a.G[(size_t)j * plane + e] = b;
+    }
+    cpa_wait<0>();
+}
+
+// slot of row j: y[j], U rows of j, and the correction operands of row j + 4 (u*, T, p, D1 p)
+struct PBwdSlot {
+    cd y[PBB];
+    double U[PWI + 1][PBB];
+    cd op[MAXF + 2][PBB];
+};
+
+__global__ void __launch_bounds__(PBB) k_poisson_bwd_correct(PoisArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PBwdSlot* slots = reinterpret_cast<PBwdSlot*>(smem_raw);
+    __shared__ cd ring[16][PBB];                        // phi of the last rows; column tx is private to thread tx
+    const int tx = threadIdx.x;
+    const int plane_i = a.M1 * a.NK;
+    const int e0 = blockIdx.x * PBB + tx;
+    const bool valid = e0 < plane_i;
+    const int e = valid ? e0 : plane_i - 1;
+    const int m = e / a.NK, kk = e % a.NK;
+    const int ka = kk >= a.K ? kk - a.K : a.K - kk;
+    const size_t P = a.P;
+    const size_t plane = (size_t)plane_i;
+    const int N = a.N_r;
+    const double n = a.nm[m], kap = a.kap[kk];
+    const bool m00 = (m == 0 && ka == 0);
+    const double idt = 1.0 / a.dt;
+    const double* Uf = a.U + (size_t)m * (a.K + 1) + ka;
+    const bool have_p = a.p_dst != nullptr;
+    const bool heated = a.nf == 4;
+    // rows whose correction operands ride in the pipeline: jc = j + 4 for j in [0, N - 9]
+    auto issue = [&](int j) {
+        if (j >= 0) {
+            PBwdSlot& s = slots[(N - 1 - j) % PIPE_PB];
+            cpa16(&s.y[tx], a.G + (size_t)j * plane + e);
+            if (j >= a.jaU && j < a.jbU) {
+                const double* Ur = Uf + (size_t)(a.offUa + (PWI + 1) * (j - a.jaU)) * P;
+#pragma unroll
+                for (int i = 0; i <= PWI; ++i) cpa8(&s.U[i][tx], Ur + (size_t)i * P);
+            }
+            if (j <= N - NPT) {
+                const size_t oc = (size_t)(j + NPT / 2) * plane + e;
+                cpa16(&s.op[0][tx], a.W[0] + oc);
+                cpa16(&s.op[1][tx], a.W[1] + oc);
+                cpa16(&s.op[2][tx], a.W[2] + oc);
+                if (a.copyT) cpa16(&s.op[3][tx], a.W[3] + oc);
+                if (have_p) {
+                    cpa16(&s.op[MAXF][tx], a.p + oc);
+                    cpa16(&s.op[MAXF + 1][tx], a.DP + oc);
+                }
+            }
+        }
+        cpa_commit();
+    };
+    // L5 at row jc from (u_r*, u_theta*, u_z*, T, p, D1 p) of that row
+    auto correct = [&](int jc, cd ur, cd ut, cd uz, cd T, cd pr, cd dp) {
+        const size_t oc = (size_t)jc * plane + e;
+        const cd phi = ring[jc & 15][tx];
+        cd gphi = mk(0.0, 0.0);
+        if (jc != 0 && jc != N - 1) {
+            const int s0 = a.s0[jc];
+            const double* d = a.D1 + jc * NPT;
+#pragma unroll
+            for (int l = 0; l < NPT; ++l) {
+                const double wt = __ldg(d + l);
+                const cd v = ring[(s0 + l) & 15][tx];
+                gphi.x = fma(wt, v.x, gphi.x);
+                gphi.y = fma(wt, v.y, gphi.y);
+            }
+        }
+        if (!valid) return;
+        const double nr = n * a.rinv[jc];
+        cd o0 = ur - gphi;
+        if (m00) o0 = mk(0.0, 0.0);
+        a.dst[0][oc] = o0;
+        a.dst[1][oc] = mk(ut.x + nr * phi.y, ut.y - nr * phi.x);          // - (i n / r) phi
+        a.dst[2][oc] = mk(uz.x + kap * phi.y, uz.y - kap * phi.x);        // - i kappa phi
+        if (a.copyT) a.dst[3][oc] = T;
+        if (have_p) {
+            a.p_dst[oc] = mk(fma(idt, phi.x, pr.x), fma(idt, phi.y, pr.y));
+            a.DP[oc] = mk(fma(idt, gphi.x, dp.x), fma(idt, gphi.y, dp.y));
+        }
+    };
+    auto correct_direct = [&](int jc) {                  // rows next to the walls: operands straight from HBM
+        const size_t oc = (size_t)jc * plane + e;
+        const cd z = mk(0.0, 0.0);
+        correct(jc, a.W[0][oc], a.W[1][oc], a.W[2][oc], a.copyT ? a.W[3][oc] : z, have_p ? a.p[oc] : z,
+                have_p ? a.DP[oc] : z);
+    };
+    cd w[PW];                                           // w[0] = phi_{j+1}
+#pragma unroll
+    for (int i = 0; i < PW; ++i) w[i] = mk(0.0, 0.0);
+#pragma unroll
+    for (int d = 0; d < PIPE_PB - 1; ++d) issue(N - 1 - d);
+    for (int j = N - 1; j >= 0; --j) {
+        cpa_wait<PIPE_PB - 2>();
+        __syncthreads();
+        issue(j - (PIPE_PB - 1));
+        const PBwdSlot& s = slots[(N - 1 - j) % PIPE_PB];
+        cd y = s.y[tx];
+        if (j >= a.jaU && j < a.jbU) {
+#pragma unroll
+            for (int q = 0; q < PWI; ++q) {
+                const double u = s.U[q + 1][tx];
+                y.x = fma(-u, w[q].x, y.x);
+                y.y = fma(-u, w[q].y, y.y);
+            }
+            y = s.U[0][tx] * y;
+        } else {
+            const int nu = a.hi[j] - j;
+            const double* Ur = Uf + (size_t)a.offU[j] * P;
+#pragma unroll
+            for (int q = 0; q < PW; ++q) {
+                if (q < nu) {
+                    const double u = Ur[(size_t)(q + 1) * P];
+                    y.x = fma(-u, w[q].x, y.x);
+                    y.y = fma(-u, w[q].y, y.y);
+                }
+            }
+            y = Ur[0] * y;
+        }
+#pragma unroll
+        for (int q = PW - 1; q > 0; --q) w[q] = w[q - 1];
+        w[0] = y;
+        ring[j & 15][tx] = y;
+        if (j == N - 1) correct_direct(N - 1);
+        if (j <= N - NPT) {
+            if (j == N - NPT)
+                for (int jc = N - 2; jc > j + NPT / 2; --jc) correct_direct(jc);
+            const cd z = mk(0.0, 0.0);
+            correct(j + NPT / 2, s.op[0][tx], s.op[1][tx], s.op[2][tx], a.copyT ? s.op[3][tx] : z,
+                    have_p ? s.op[MAXF][tx] : z, have_p ? s.op[MAXF + 1][tx] : z);
+            if (j == 0)
+                for (int jc = NPT / 2 - 1; jc >= 0; --jc) correct_direct(jc);
+        }
+    }
+    cpa_wait<0>();
+    (void)heated;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -763,6 +1016,26 @@ static int run_solve(nsc_ctx* c, const BandFactors& f, const BandShape& s, cd* x
     return NSC_OK;
 }
 
+// longest run [ja, jb) of rows whose lower (upper) width equals `width`; off = offL[ja] (offU[ja])
+static void interior_run(const BandShape& s, bool lower, int width, int& ja, int& jb, int& off) {
+    const int N = (int)s.h_lo.size();
+    int best_a = 0, best_b = 0, cur = -1;
+    for (int j = 0; j <= N; ++j) {
+        const bool in = j < N && (lower ? j - s.h_lo[j] : s.h_hi[j] - j) == width;
+        if (in && cur < 0) cur = j;
+        if (!in && cur >= 0) {
+            if (j - cur > best_b - best_a) {
+                best_a = cur;
+                best_b = j;
+            }
+            cur = -1;
+        }
+    }
+    ja = best_a;
+    jb = best_b;
+    off = (best_b > best_a) ? (lower ? s.h_offL[best_a] : s.h_offU[best_a]) : 0;
+}
+
 int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w1, double dt, cd* const* dst,
                    cd* p_dst) {
     int rc = ensure_factors(c, dt);
@@ -839,29 +1112,68 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
         fa.offU4 = c->shH.h_offU[FWI];
         static bool attr_done = false;
         if (!attr_done) {
-            cudaFuncSetAttribute(k_rhs_fwd<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE * sizeof(FwdSlot<3>)));
-            cudaFuncSetAttribute(k_rhs_fwd<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE * sizeof(FwdSlot<4>)));
-            cudaFuncSetAttribute(k_bwd_div<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE * sizeof(BwdSlot<3>)));
-            cudaFuncSetAttribute(k_bwd_div<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE * sizeof(BwdSlot<4>)));
+            cudaFuncSetAttribute(k_rhs_fwd<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_F * sizeof(FwdSlot<3>)));
+            cudaFuncSetAttribute(k_rhs_fwd<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_F * sizeof(FwdSlot<4>)));
+            cudaFuncSetAttribute(k_bwd_div<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_B * sizeof(BwdSlot<3>)));
+            cudaFuncSetAttribute(k_bwd_div<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_B * sizeof(BwdSlot<4>)));
             attr_done = true;
         }
         prof_begin(c, NSC_K_RHS);
         if (c->nf == 3)
-            k_rhs_fwd<3><<<nb, dim3(PBK, 3), PIPE * sizeof(FwdSlot<3>), c->stream>>>(fa);
+            k_rhs_fwd<3><<<nb, dim3(PBK, 3), PIPE_F * sizeof(FwdSlot<3>), c->stream>>>(fa);
         else
-            k_rhs_fwd<4><<<nb, dim3(PBK, 4), PIPE * sizeof(FwdSlot<4>), c->stream>>>(fa);
+            k_rhs_fwd<4><<<nb, dim3(PBK, 4), PIPE_F * sizeof(FwdSlot<4>), c->stream>>>(fa);
         prof_end(c);
         NSC_CUDA(c, cudaGetLastError());
         prof_begin(c, NSC_K_HELMHOLTZ);
         if (c->nf == 3)
-            k_bwd_div<3><<<nb, dim3(PBK, 4), PIPE * sizeof(BwdSlot<3>), c->stream>>>(fa);
+            k_bwd_div<3><<<nb, dim3(PBK, 4), PIPE_B * sizeof(BwdSlot<3>), c->stream>>>(fa);
         else
-            k_bwd_div<4><<<nb, dim3(PBK, 5), PIPE * sizeof(BwdSlot<4>), c->stream>>>(fa);
+            k_bwd_div<4><<<nb, dim3(PBK, 5), PIPE_B * sizeof(BwdSlot<4>), c->stream>>>(fa);
         prof_end(c);
         NSC_CUDA(c, cudaGetLastError());
-        if ((rc = run_solve(c, c->facP, c->shP, c->G, true))) return rc;
+        PoisArgs pa{};
+        pa.G = c->G;
+        pa.L = c->facP.L;
+        pa.U = c->facP.U;
+        pa.lo = c->shP.lo;
+        pa.hi = c->shP.hi;
+        pa.offL = c->shP.offL;
+        pa.offU = c->shP.offU;
+        interior_run(c->shP, true, PWI, pa.jaL, pa.jbL, pa.offLa);
+        interior_run(c->shP, false, PWI, pa.jaU, pa.jbU, pa.offUa);
+        for (int i = 0; i < c->nf; ++i) {
+            pa.W[i] = c->W[i];
+            pa.dst[i] = dst[i];
+        }
+        pa.p = c->state[4];
+        pa.p_dst = p_dst;
+        pa.DP = c->DP;
+        pa.D1 = c->t.D1;
+        pa.rinv = c->t.rinv;
+        pa.nm = c->t.nm;
+        pa.kap = c->t.kap;
+        pa.s0 = c->t.s0;
+        pa.N_r = c->N_r;
+        pa.M1 = c->M1;
+        pa.NK = c->NK;
+        pa.K = c->K;
+        pa.P = c->P;
+        pa.nf = c->nf;
+        pa.copyT = (c->nf == 4 && dst[3] != c->W[3]) ? 1 : 0;
+        pa.dt = dt;
+        static bool pattr_done = false;
+        if (!pattr_done) {
+            cudaFuncSetAttribute(k_poisson_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_PF * sizeof(PFwdSlot)));
+            cudaFuncSetAttribute(k_poisson_bwd_correct, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_PB * sizeof(PBwdSlot)));
+            pattr_done = true;
+        }
+        prof_begin(c, NSC_K_POISSON);
+        k_poisson_fwd<<<(plane + PBP - 1) / PBP, PBP, PIPE_PF * sizeof(PFwdSlot), c->stream>>>(pa);
+        prof_end(c);
+        NSC_CUDA(c, cudaGetLastError());
         prof_begin(c, NSC_K_CORRECT);
-        k_correct<<<gridp, 128, 0, c->stream>>>(a);
+        k_poisson_bwd_correct<<<(plane + PBB - 1) / PBB, PBB, PIPE_PB * sizeof(PBwdSlot), c->stream>>>(pa);
         prof_end(c);
         NSC_CUDA(c, cudaGetLastError());
         return NSC_OK;
