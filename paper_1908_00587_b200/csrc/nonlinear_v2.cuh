@@ -333,18 +333,19 @@ struct SmemScratch {
 };
 
 template <bool TMEM> struct T2Cfg;
+constexpr int T2_STAGE = 264;      // complex elements of one staged half-spectral line (>= M + 1 = 257)
 template <> struct T2Cfg<true> {
     static constexpr int WARPS = 8;
     using Scratch = TmemScratch;
-    // the request is padded above half of the SM's shared memory so that exactly one CTA (the owner
-    // of all 512 TMEM columns) is resident per SM
-    static constexpr size_t SMEM = 120 * 1024;
+    // twiddles + one exchange matrix and one staged line pair per warp; more than half of the SM's
+    // shared memory, so exactly one CTA (the owner of all 512 TMEM columns) is resident per SM
+    static constexpr size_t SMEM = sizeof(cd) * ((size_t)f768::XBUF * (1 + WARPS) + (size_t)2 * T2_STAGE * WARPS);
 };
 template <> struct T2Cfg<false> {
     static constexpr int WARPS = 5;
     using Scratch = SmemScratch;
-    static constexpr size_t SMEM =
-        sizeof(cd) * (size_t)f768::XBUF * (1 + WARPS) + sizeof(double) * (size_t)WARPS * T2_NSLOT * 32 * f768::NA;
+    static constexpr size_t SMEM = sizeof(cd) * ((size_t)f768::XBUF * (1 + WARPS) + (size_t)2 * T2_STAGE * WARPS) +
+                                   sizeof(double) * (size_t)WARPS * T2_NSLOT * 32 * f768::NA;
 };
 
 // chunked access (8 doubles = elements 8 c .. 8 c + 7 of a slot)
@@ -530,7 +531,7 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         sc.base = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 256);
     } else {
-        double* sb = reinterpret_cast<double*>(tw + XBUF * (1 + Cfg::WARPS));
+        double* sb = reinterpret_cast<double*>(tw + XBUF * (1 + Cfg::WARPS) + 2 * T2_STAGE * Cfg::WARPS);
         sc.base = sb + (size_t)warp * T2_NSLOT * 32 * NA + a23;
         sc.active = tau < NA;
         __syncthreads();
@@ -540,27 +541,37 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
     const size_t qstride = (size_t)a.JC * a.Nz * a.MP;
     const int nlines = a.nj * a.Nz;
     const int lstride = gridDim.x * Cfg::WARPS;
-    for (int line = blockIdx.x * Cfg::WARPS + warp; line < nlines; line += lstride) {
+    // this warp's staged line pair (X, Y) of the next inverse transform, filled by cp.async
+    cd* stX = tw + XBUF * (1 + Cfg::WARPS) + 2 * T2_STAGE * warp;
+    cd* stY = stX + T2_STAGE;
+    auto stage = [&](int ln, int t) {
+        const size_t off = (size_t)ln * a.MP;
+        const cd* X = a.zbuf + (size_t)t2_qx(t) * qstride + off;
+        const cd* Y = a.zbuf + (size_t)t2_qy(t) * qstride + off;
+        for (int i = tau; i <= M; i += 32) {
+            cp_async16(stX + i, X + i);
+            cp_async16(stY + i, Y + i);
+        }
+    };
+    int line = blockIdx.x * Cfg::WARPS + warp;
+    if (line < nlines) stage(line, 0);
+    for (; line < nlines; line += lstride) {
         const int jl = line / a.Nz;
         const size_t loff = (size_t)line * a.MP;               // (jl * Nz + z) * MP
         const double ri = a.rinv[a.j0 + jl];
         const double rj = 1.0 / ri;
-        if (line + lstride < nlines) {                         // next line's nine inputs -> L2
-            const size_t noff = (size_t)(line + lstride) * a.MP;
-#pragma unroll
-            for (int q = 0; q < 9; ++q) {
-                const char* p = reinterpret_cast<const char*>(a.zbuf + (size_t)q * qstride + noff);
-                prefetch_l2(p + tau * 128);
-                if (tau == 0) prefetch_l2(p + 32 * 128);
-            }
-        }
         cd x[32];
         double acc[32];
 #pragma unroll 1
         for (int t = 0; t < 6; ++t) {
-            const cd* X = a.zbuf + (size_t)t2_qx(t) * qstride + loff;
-            const cd* Y = a.zbuf + (size_t)t2_qy(t) * qstride + loff;
-            load_pair768_rt(x, X, Y, t == 2 || t == 5, t == 3, M, tau, taud, kth0);
+            cp_async_commit_wait_all();
+            __syncwarp();
+            load_pair768_rt(x, stX, stY, t == 2 || t == 5, t == 3, M, tau, taud, kth0);
+            __syncwarp();                                      // the staged pair is consumed: request the next one
+            if (t < 5)
+                stage(line, t + 1);
+            else if (line + lstride < nlines)
+                stage(line + lstride, 0);
             s2p<+1>(x, buf, tw, tau);
             sc_fence(sc);
             // physical-space stage (N4): slots 0 U_r, 1 U_theta / r, 2 U_z, 3 parked line
@@ -651,6 +662,7 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
             }
         }
     }
+    cp_async_commit_wait_all();
     if constexpr (TMEM) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
