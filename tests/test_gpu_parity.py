@@ -178,3 +178,43 @@ def test_host_buffer_entry_points_and_errors(torch_cuda):
         assert ctx.launch_count() == n0
         ctx.step(1e-3)
         assert ctx.launch_count() > n0
+
+
+def test_full_size_cfg4_sampled(torch_cuda):
+    """BASELINE.json configs[3] at full size (N_r = 256, M = K = 256, 768 x 768 grid), in the launch
+    configuration bench.py times (length-768 transform pipeline + fused linear sweeps): the nonlinear
+    term at sampled radial nodes and one sub-step at sampled modes against the oracle, then the
+    divergence of the stepped state at round-off (a property that holds at any size)."""
+    torch = torch_cuda
+    cfg = synth.config(3)
+    o = oracle_of(cfg, dft="fft")
+    nodes = [0, 1, 4, 127, 200, 251, 254, 255]
+    rng = np.random.default_rng(11)
+    im = np.concatenate([[0, 0, 0, cfg["M"], cfg["M"], 1], rng.integers(0, cfg["M"] + 1, 26)])
+    ik = np.concatenate([[cfg["K"], cfg["K"] + 1, 0, 0, 2 * cfg["K"], cfg["K"] - 1], rng.integers(0, 2 * cfg["K"] + 1, 26)])
+    with _ctx(cfg) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        got = ctx.nonlinear_to_host()
+        ref = o.nonlinear(*st[:3], nodes=nodes)
+        assert rel_l2([g[nodes] for g in got], ref) <= TOL_N
+        # sub-step with the nonlinear term just computed as the explicit term
+        E = got
+        ctx.substep(*_dev(torch, E), None, cfg["dt"])
+        sub = ctx.state_to_host()
+        ref_s = o.substep(st, E, cfg["dt"], modes=(im, ik))
+        got_s = [f[:, im, ik] for f in sub[:3]]
+        assert rel_l2(got_s, ref_s[:3]) <= TOL_STEP
+        # scaled divergence of the new state (formula of SURVEY.md section 8(c), pin T5)
+        ur, ut, uz = sub[:3]
+        r = o.r[:, None, None]
+        n = o.n[None, :, None]
+        kap = o.kappa[None, None, :]
+        d = o.divergence(ur, ut, uz)[1:-1]
+        scale = (np.abs(o.D1) @ np.abs(ur).reshape(cfg["N_r"], -1)).reshape(ur.shape) + np.abs(ur) / r \
+            + np.abs(n / r * ut) + np.abs(kap * uz)
+        scale = scale[1:-1]
+        mask = scale > 0
+        # SURVEY T5 quotes <= 1e-9 for single modes at N_r = 256; over all 3.3e7 interior mode-points of the
+        # broadband state the maximum is a few 1e-9 (cond(P) ~ 1e13 on the Chebyshev grid): bar 1e-8
+        assert np.max(np.abs(d[mask]) / scale[mask]) <= 1e-8
