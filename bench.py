@@ -80,8 +80,26 @@ def flops_per_nonlinear(cfg):
     return inv + fwd + N_r * Nt * Nz * (22 if nf == 3 else 30)
 
 
-LINEAR_KERNELS = ("k_rhs", "k_band_solve<helmholtz>", "k_recombine", "k_div", "k_band_solve<poisson>",
-                  "k_correct", "k_linear")
+LINEAR_KERNELS = ("k_rhs_fwd", "k_bwd_div", "k_poisson_fwd", "k_poisson_bwd_correct")
+
+# fp64 peak of the plain DFMA pipe: 148 SM x 64 lanes x 2 flop x 1.965 GHz
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/r01_ncu_full.md), cfg 4, full 55-level radial chunk; None where no capture exists
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {
+    ("k_theta", 4): 2.984962e9 + 0.599447e9,
+    ("k_zinv", 4): 0.696536e9 + 1.554002e9,
+}
+
+
+def flops_theta_per_nonlinear(cfg):
+    """The theta kernel's share of flops_per_nonlinear: 4 nf inverse + nf forward real lines of length
+    N_theta per (j, z) point-line (2.5 N log2 N each) + the physical-space products."""
+    import math
+    s = sizes(cfg)
+    tl = 2.5 * s["Nt"] * math.log2(s["Nt"])
+    return s["N_r"] * s["Nz"] * (5 * s["nf"] * tl + s["Nt"] * (22 if s["nf"] == 3 else 30))
 
 
 # ------------------------------------------------------------------------------------------
@@ -369,7 +387,8 @@ def run_ours(args, cfg, rank, world, local_rank):
     launches_dom = dom.get("launches_per_step", None)
     roofline = {
         "bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_GBs"], "peak": peak, "unit": "GB/s",
-        "frac": dom["achieved_GBs"] / peak, "peak_source": peak_src, "traffic": None,
+        "frac": dom["achieved_GBs"] / peak, "peak_source": peak_src,
+        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((dom["kernel"], args.config)),
         "share_of_step": dom["share"],
         "algorithmic_bytes_per_launch": (model.get(dom["kernel"], model["linear"]) / launches_dom
                                          if launches_dom else None),
@@ -378,6 +397,12 @@ def run_ours(args, cfg, rank, world, local_rank):
                  "frac_of_measured": model["step"] / 1e6 / ms_per_step / peak,
                  "frac_of_nominal_8TBs": model["step"] / 1e6 / ms_per_step / NOMINAL_HBM_GBS},
         "fp64": {"GF_per_nonlinear": flops_per_nonlinear(cfg) / 1e9},
+        # the theta kernel is co-bound by the plain fp64 pipe: its own ALU roofline
+        "alu": ({"kernel": "k_theta", "achieved": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"],
+                 "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                 "frac": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"] / FP64_PEAK_TFLOPS,
+                 "peak_source": "148 SM x 64 DFMA lanes x 2 x 1.965 GHz (nominal)"}
+                if (th := next((k for k in kern if k["kernel"] == "k_theta"), None)) else None),
         "kernels": kern + [lin],
         "ms_per_step_with_event_brackets": ms_prof_per_step,
     }

@@ -131,12 +131,12 @@ enum {
     NSC_K_ZINV = 0,      /* N1 + N2: z-derivative, radial derivative, padded inverse z-FFT          */
     NSC_K_THETA = 1,     /* N1 + N3 + N4 + N5: fused theta transforms and physical-space products   */
     NSC_K_ZFWD = 2,      /* N6: forward z-FFT, truncation, scaling, buoyancy                         */
-    NSC_K_RHS = 3,       /* L1                                                                       */
-    NSC_K_HELMHOLTZ = 4, /* L2: banded solves for u_+, u_-, u_z, T                                  */
-    NSC_K_RECOMBINE = 5, /* L3a                                                                      */
-    NSC_K_DIV = 6,       /* L3b                                                                      */
-    NSC_K_POISSON = 7,   /* L4                                                                       */
-    NSC_K_CORRECT = 8,   /* L5                                                                       */
+    NSC_K_RHS = 3,       /* L1 + L2 (k_rhs_fwd): right-hand sides + forward substitution, marching up   */
+    NSC_K_HELMHOLTZ = 4, /* L2 + L3 (k_bwd_div): back substitution, recombination, divergence, down     */
+    NSC_K_RECOMBINE = 5, /* (unused: fused into k_bwd_div)                                               */
+    NSC_K_DIV = 6,       /* (unused: fused into k_bwd_div)                                               */
+    NSC_K_POISSON = 7,   /* L4 (k_poisson_fwd): forward substitution of the pressure system, up          */
+    NSC_K_CORRECT = 8,   /* L4 + L5 (k_poisson_bwd_correct): back substitution + correction, down        */
     NSC_K_FACTOR = 9,    /* set-up: banded LU of the per-mode matrices (once per dt)                 */
     NSC_K_DR = 10,       /* N1: radial derivative of the spectral fields (length-768 pipeline only)  */
     NSC_NKERN = 11

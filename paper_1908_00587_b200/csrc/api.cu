@@ -65,8 +65,8 @@ void prof_end(nsc_ctx* c) {
     cudaEventRecord(c->prof.back().b, c->stream);
 }
 
-static const char* kKernelNames[NSC_NKERN] = {"k_zinv", "k_theta", "k_zfwd", "k_rhs", "k_band_solve<helmholtz>",
-                                              "k_recombine", "k_div", "k_band_solve<poisson>", "k_correct",
+static const char* kKernelNames[NSC_NKERN] = {"k_zinv", "k_theta", "k_zfwd", "k_rhs_fwd", "k_bwd_div",
+                                              "(unused)", "(unused)", "k_poisson_fwd", "k_poisson_bwd_correct",
                                               "k_factor", "k_dr"};
 
 static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
@@ -138,7 +138,6 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
         c->t768 = (c->Nt == 768 && c->M <= 256 && c->nf == 3) ? ((variant >> 1) & 3) : 0;
         if (c->t768 > 2) c->t768 = 2;
     }
-    if (const char* ev = getenv("NSC_LIN_VARIANT")) c->lin_fused = atoi(ev) != 0;
     int rc = build_plan(c);
     if (!rc && c->z768)
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->DR[i], c->F, false);
@@ -149,7 +148,7 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->N0[i], c->F, false);
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->N1[i], c->F, false);
         if (!rc) rc = dev_alloc(c, &c->G, c->F, false);
-        if (!rc && c->lin_fused) rc = dev_alloc(c, &c->DP, c->F, true);
+        if (!rc) rc = dev_alloc(c, &c->DP, c->F, true);
         if (!rc) rc = dev_alloc(c, &c->zbuf, (size_t)3 * c->nf * c->JC * c->Nz * c->MP, true);
         if (!rc) rc = dev_alloc(c, &c->tbuf, (size_t)c->nf * c->JC * c->Nz * c->MP, true);
     }

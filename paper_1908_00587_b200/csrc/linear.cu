@@ -7,9 +7,11 @@
 // Per-mode matrices differ from mode to mode only on the diagonal:
 //   Helmholtz  A = I - coef (L0 - diag((n + shift)^2 / r^2 + kappa^2)),  identity rows at the walls
 //   Poisson    P = Q - diag(n^2 / r^2 + kappa^2),  Neumann rows D1[wall] at the walls (R9)
-// and are the same for +k and -k, so one thread serves the pair (m, |k|).  They are LU-factored
-// without pivoting inside their row envelope (no fill-in outside it) once per dt (Helmholtz) /
-// once per context (Poisson); the solves stream the factors with pair-major (coalesced) access.
+// and are the same for +k and -k.  They are LU-factored without pivoting inside their row envelope
+// (no fill-in outside it) once per dt (Helmholtz) / once per context (Poisson), pair-major
+// ("pair" = (m, |k|)).  The sub-step is four marching sweeps over the radial index, one thread per
+// (mode, field), every row's operands prefetched into shared memory by a cp.async row pipeline:
+//   k_rhs_fwd (up) -> k_bwd_div (down) -> k_poisson_fwd (up) -> k_poisson_bwd_correct (down).
 #include <cstdint>
 #include "nsc_internal.h"
 
@@ -87,266 +89,13 @@ __global__ void k_factor(FacArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------
-// banded solve, in place, both modes (m, +k) and (m, -k) of a pair per thread
-struct SolveArgs {
-    const double* L;
-    const double* U;
-    const int *lo, *hi, *offL, *offU;
-    cd* x;              // [N_r][M1][NK]
-    int N_r, M1, NK, K, P;
-};
-
-template <int WREG, int WMAX>
-__global__ void __launch_bounds__(128) k_band_solve(SolveArgs a) {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= a.P) return;
-    const int m = p / (a.K + 1), ka = p % (a.K + 1);
-    const size_t P = a.P;
-    const size_t plane = (size_t)a.M1 * a.NK;
-    cd* xp = a.x + (size_t)m * a.NK + a.K + ka;
-    cd* xm = a.x + (size_t)m * a.NK + a.K - ka;
-    cd wp[WMAX], wm[WMAX];                      // w[WMAX-1] = most recent row
-#pragma unroll
-    for (int i = 0; i < WMAX; ++i) wp[i] = wm[i] = mk(0.0, 0.0);
-    // forward: y_j = b_j - sum_i L[j][i] y_{lo+i}
-    for (int j = 0; j < a.N_r; ++j) {
-        const int nl = j - a.lo[j];
-        const double* Lr = a.L + (size_t)a.offL[j] * P + p;
-        cd bp = xp[(size_t)j * plane], bm = xm[(size_t)j * plane];
-        if (nl == WREG) {
-#pragma unroll
-            for (int q = WMAX - WREG; q < WMAX; ++q) {
-                const double l = Lr[(size_t)(q - (WMAX - WREG)) * P];
-                bp.x = fma(-l, wp[q].x, bp.x);
-                bp.y = fma(-l, wp[q].y, bp.y);
-                bm.x = fma(-l, wm[q].x, bm.x);
-                bm.y = fma(-l, wm[q].y, bm.y);
-            }
-        } else {
-#pragma unroll
-            for (int q = 0; q < WMAX; ++q) {
-                const int i = q - (WMAX - nl);
-                if (i >= 0) {
-                    const double l = Lr[(size_t)i * P];
-                    bp.x = fma(-l, wp[q].x, bp.x);
-                    bp.y = fma(-l, wp[q].y, bp.y);
-                    bm.x = fma(-l, wm[q].x, bm.x);
-                    bm.y = fma(-l, wm[q].y, bm.y);
-                }
-            }
-        }
-#pragma unroll
-        for (int q = 0; q < WMAX - 1; ++q) {
-            wp[q] = wp[q + 1];
-            wm[q] = wm[q + 1];
-        }
-        wp[WMAX - 1] = bp;
-        wm[WMAX - 1] = bm;
-        xp[(size_t)j * plane] = bp;
-        if (ka != 0) xm[(size_t)j * plane] = bm;
-    }
-    // backward: x_j = (y_j - sum_{i>=1} U[j][i] x_{j+i}) / pivot;  w[0] = x_{j+1}
-    for (int j = a.N_r - 1; j >= 0; --j) {
-        const int nu = a.hi[j] - j;
-        const double* Ur = a.U + (size_t)a.offU[j] * P + p;
-        cd yp = xp[(size_t)j * plane], ym = xm[(size_t)j * plane];
-        if (nu == WREG) {
-#pragma unroll
-            for (int q = 0; q < WREG; ++q) {
-                const double u = Ur[(size_t)(q + 1) * P];
-                yp.x = fma(-u, wp[q].x, yp.x);
-                yp.y = fma(-u, wp[q].y, yp.y);
-                ym.x = fma(-u, wm[q].x, ym.x);
-                ym.y = fma(-u, wm[q].y, ym.y);
-            }
-        } else {
-#pragma unroll
-            for (int q = 0; q < WMAX; ++q) {
-                if (q < nu) {
-                    const double u = Ur[(size_t)(q + 1) * P];
-                    yp.x = fma(-u, wp[q].x, yp.x);
-                    yp.y = fma(-u, wp[q].y, yp.y);
-                    ym.x = fma(-u, wm[q].x, ym.x);
-                    ym.y = fma(-u, wm[q].y, ym.y);
-                }
-            }
-        }
-        const double dinv = Ur[0];
-        yp = dinv * yp;
-        ym = dinv * ym;
-#pragma unroll
-        for (int q = WMAX - 1; q > 0; --q) {
-            wp[q] = wp[q - 1];
-            wm[q] = wm[q - 1];
-        }
-        wp[0] = yp;
-        wm[0] = ym;
-        xp[(size_t)j * plane] = yp;
-        if (ka != 0) xm[(size_t)j * plane] = ym;
-    }
-}
-
-// ------------------------------------------------------------------------------------------
-// element-wise / stencil kernels
-struct LinArgs {
-    const cd* u[MAXF];     // state n: u_r, u_theta, u_z, T
-    const cd* p;           // pressure n
-    const cd* E0[MAXF];
-    const cd* E1[MAXF];    // may be null
-    cd* W[MAXF];           // work: rhs_+ / rhs_- / rhs_z / rhs_T  ->  u_r*, u_theta*, u_z*, T
-    cd* G;                 // divergence / phi
-    cd* dst[MAXF];         // corrected fields
-    cd* p_dst;             // new pressure (may be null)
-    cd* DP;                // D1 p, updated with D1 phi / dt when p_dst is set (may be null)
-    const double *D1, *L0, *rinv, *nm, *kap;
-    const int* s0;
-    int N_r, M1, NK, K, nf;
-    double dt, c, w0, w1, inv_Pr, Re_i, Re_o;
-};
-
-// L1: rhs_+- = u_+- + dt[(1-c) L_+- u_+- + E_+- - (D1 p -+ (n/r) p)],  rhs_z, rhs_T likewise;
-// wall rows carry the Dirichlet data (R1).
-__global__ void __launch_bounds__(128) k_rhs(LinArgs a) {
-    const int plane = a.M1 * a.NK;
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= plane) return;
-    const int j = blockIdx.y;
-    const int m = e / a.NK, kk = e % a.NK;
-    const size_t o = (size_t)j * plane + e;
-    const bool heated = a.nf == 4;
-    if (j == 0 || j == a.N_r - 1) {
-        const bool m00 = (m == 0 && kk == a.K);
-        const double v = m00 ? (j == 0 ? a.Re_i : a.Re_o) : 0.0;
-        a.W[0][o] = mk(0.0, v);                 // u_+ = u_r + i u_theta = i Re
-        a.W[1][o] = mk(0.0, -v);
-        a.W[2][o] = mk(0.0, 0.0);
-        if (heated) a.W[3][o] = mk(m00 ? (j == 0 ? 0.5 : -0.5) : 0.0, 0.0);
-        return;
-    }
-    const int s = a.s0[j];
-    cd Sr = mk(0, 0), St = mk(0, 0), Sz = mk(0, 0), ST = mk(0, 0), Dp = mk(0, 0);
-#pragma unroll
-    for (int l = 0; l < NPT; ++l) {
-        const size_t ol = (size_t)(s + l) * plane + e;
-        const double wl = a.L0[j * NPT + l], wd = a.D1[j * NPT + l];
-        cd v = a.u[0][ol];
-        Sr.x = fma(wl, v.x, Sr.x);
-        Sr.y = fma(wl, v.y, Sr.y);
-        v = a.u[1][ol];
-        St.x = fma(wl, v.x, St.x);
-        St.y = fma(wl, v.y, St.y);
-        v = a.u[2][ol];
-        Sz.x = fma(wl, v.x, Sz.x);
-        Sz.y = fma(wl, v.y, Sz.y);
-        if (heated) {
-            v = a.u[3][ol];
-            ST.x = fma(wl, v.x, ST.x);
-            ST.y = fma(wl, v.y, ST.y);
-        }
-        v = a.p[ol];
-        Dp.x = fma(wd, v.x, Dp.x);
-        Dp.y = fma(wd, v.y, Dp.y);
-    }
-    const double ri = a.rinv[j], n = a.nm[m], kap = a.kap[kk];
-    const double k2 = kap * kap, r2 = ri * ri;
-    const double qp = (n + 1) * (n + 1) * r2 + k2, qm = (n - 1) * (n - 1) * r2 + k2, q0 = n * n * r2 + k2;
-    const cd ur = a.u[0][o], ut = a.u[1][o], uz = a.u[2][o], pr = a.p[o];
-    cd Er = a.w0 * a.E0[0][o], Et = a.w0 * a.E0[1][o], Ez = a.w0 * a.E0[2][o];
-    if (a.E1[0]) {
-        Er = Er + a.w1 * a.E1[0][o];
-        Et = Et + a.w1 * a.E1[1][o];
-        Ez = Ez + a.w1 * a.E1[2][o];
-    }
-    const double omc = 1.0 - a.c, dt = a.dt;
-    const cd up = ur + mul_i(ut), um = ur - mul_i(ut);
-    const cd Lp = (Sr + mul_i(St)) - qp * up, Lm = (Sr - mul_i(St)) - qm * um;
-    const cd npr = (n * ri) * pr;
-    a.W[0][o] = up + dt * (omc * Lp + (Er + mul_i(Et)) - (Dp - npr));
-    a.W[1][o] = um + dt * (omc * Lm + (Er - mul_i(Et)) - (Dp + npr));
-    a.W[2][o] = uz + dt * (omc * (Sz - q0 * uz) + Ez - kap * mul_i(pr));
-    if (heated) {
-        const cd T = a.u[3][o];
-        cd ET = a.w0 * a.E0[3][o];
-        if (a.E1[3]) ET = ET + a.w1 * a.E1[3][o];
-        a.W[3][o] = T + dt * ((omc * a.inv_Pr) * (ST - q0 * T) + ET);
-    }
-}
-
-// L3a: u_r* = (u_+ + u_-)/2, u_theta* = (u_+ - u_-)/(2i), in place in W[0], W[1]
-__global__ void __launch_bounds__(256) k_recombine(LinArgs a, size_t total) {
-    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= total) return;
-    const cd up = a.W[0][o], um = a.W[1][o];
-    a.W[0][o] = 0.5 * (up + um);
-    a.W[1][o] = 0.5 * mul_mi(up - um);
-}
-
-// L3b: g = D1 u_r* + u_r*/r + (i n / r) u_theta* + i kappa u_z*;  g = 0 in the wall rows
-__global__ void __launch_bounds__(128) k_div(LinArgs a) {
-    const int plane = a.M1 * a.NK;
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= plane) return;
-    const int j = blockIdx.y;
-    const size_t o = (size_t)j * plane + e;
-    if (j == 0 || j == a.N_r - 1) {
-        a.G[o] = mk(0.0, 0.0);
-        return;
-    }
-    const int m = e / a.NK, kk = e % a.NK;
-    const int s = a.s0[j];
-    cd d = mk(0, 0);
-#pragma unroll
-    for (int l = 0; l < NPT; ++l) {
-        const double wd = a.D1[j * NPT + l];
-        const cd v = a.W[0][(size_t)(s + l) * plane + e];
-        d.x = fma(wd, v.x, d.x);
-        d.y = fma(wd, v.y, d.y);
-    }
-    const double ri = a.rinv[j];
-    a.G[o] = d + ri * a.W[0][o] + (a.nm[m] * ri) * mul_i(a.W[1][o]) + a.kap[kk] * mul_i(a.W[2][o]);
-}
-
-// L5: u = u* - (G~ phi, (i n / r) phi, i kappa phi);  p_new = p + phi / dt;  u_r(0,0) := 0 (O8)
-__global__ void __launch_bounds__(128) k_correct(LinArgs a) {
-    const int plane = a.M1 * a.NK;
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= plane) return;
-    const int j = blockIdx.y;
-    const size_t o = (size_t)j * plane + e;
-    const int m = e / a.NK, kk = e % a.NK;
-    cd gphi = mk(0, 0);
-    if (j != 0 && j != a.N_r - 1) {
-        const int s = a.s0[j];
-#pragma unroll
-        for (int l = 0; l < NPT; ++l) {
-            const double wd = a.D1[j * NPT + l];
-            const cd v = a.G[(size_t)(s + l) * plane + e];
-            gphi.x = fma(wd, v.x, gphi.x);
-            gphi.y = fma(wd, v.y, gphi.y);
-        }
-    }
-    const cd phi = a.G[o];
-    const double ri = a.rinv[j];
-    cd ur = a.W[0][o] - gphi;
-    if (m == 0 && kk == a.K) ur = mk(0.0, 0.0);
-    a.dst[0][o] = ur;
-    a.dst[1][o] = a.W[1][o] - (a.nm[m] * ri) * mul_i(phi);
-    a.dst[2][o] = a.W[2][o] - a.kap[kk] * mul_i(phi);
-    if (a.nf == 4 && a.dst[3] != a.W[3]) a.dst[3][o] = a.W[3][o];
-    if (a.p_dst) {
-        a.p_dst[o] = a.p[o] + (1.0 / a.dt) * phi;
-        if (a.DP) a.DP[o] = a.DP[o] + (1.0 / a.dt) * gphi;
-    }
-}
-
-// ------------------------------------------------------------------------------------------
-// Fused sweeps (default path).  One thread serves one (mode, field): field 0 u_+, 1 u_-, 2 u_z, 3 T;
+// Fused sweeps.  One thread serves one (mode, field): field 0 u_+, 1 u_-, 2 u_z, 3 T;
 // the factors of the pair (m, |k|) are read by both of its modes (the second read hits L2).
 //
 // With A = I - c dt nu L and gamma = (1 - c) / c the right-hand side of step L1 is
 //     u + dt (1 - c) nu L u + dt R  =  u / c - gamma A u + dt R        (R = E - pressure-gradient term),
 // so   x = A^-1 (u / c + dt R) - gamma u   at interior rows: no radial stencil acts on u.  D1 p is kept
-// as an array of its own (DP), updated by k_correct with D1 phi / dt (D1 is linear).  Wall rows of A are identity rows: b_wall = BC + gamma u_wall.
+// as an array of its own (DP), updated by k_poisson_bwd_correct with D1 phi / dt (D1 is linear).  Wall rows of A are identity rows: b_wall = BC + gamma u_wall.
 //
 //   k_rhs_fwd  (marching up)   : b from u, E, p, D1 p, forward
 //                                substitution with the stored L factors, y -> W[field]
@@ -990,32 +739,6 @@ int ensure_factors(nsc_ctx* c, double dt) {
     return NSC_OK;
 }
 
-static int run_solve(nsc_ctx* c, const BandFactors& f, const BandShape& s, cd* x, bool poisson) {
-    SolveArgs a{};
-    a.L = f.L;
-    a.U = f.U;
-    a.lo = s.lo;
-    a.hi = s.hi;
-    a.offL = s.offL;
-    a.offU = s.offU;
-    a.x = x;
-    a.N_r = c->N_r;
-    a.M1 = c->M1;
-    a.NK = c->NK;
-    a.K = c->K;
-    a.P = c->P;
-    const int threads = 128;
-    const int blocks = (c->P + threads - 1) / threads;
-    prof_begin(c, poisson ? NSC_K_POISSON : NSC_K_HELMHOLTZ);
-    if (poisson)
-        k_band_solve<8, 12><<<blocks, threads, 0, c->stream>>>(a);
-    else
-        k_band_solve<4, 8><<<blocks, threads, 0, c->stream>>>(a);
-    prof_end(c);
-    NSC_CUDA(c, cudaGetLastError());
-    return NSC_OK;
-}
-
 // longest run [ja, jb) of rows whose lower (upper) width equals `width`; off = offL[ja] (offU[ja])
 static void interior_run(const BandShape& s, bool lower, int width, int& ja, int& jb, int& off) {
     const int N = (int)s.h_lo.size();
@@ -1040,39 +763,8 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
                    cd* p_dst) {
     int rc = ensure_factors(c, dt);
     if (rc) return rc;
-    LinArgs a{};
-    for (int i = 0; i < c->nf; ++i) {
-        a.u[i] = c->state[i];
-        a.E0[i] = E0[i];
-        a.E1[i] = E1 ? E1[i] : nullptr;
-        a.W[i] = c->W[i];
-        a.dst[i] = dst[i];
-    }
-    a.p = c->state[4];
-    a.G = c->G;
-    a.p_dst = p_dst;
-    a.DP = c->lin_fused ? c->DP : nullptr;
-    a.D1 = c->t.D1;
-    a.L0 = c->t.L0;
-    a.rinv = c->t.rinv;
-    a.nm = c->t.nm;
-    a.kap = c->t.kap;
-    a.s0 = c->t.s0;
-    a.N_r = c->N_r;
-    a.M1 = c->M1;
-    a.NK = c->NK;
-    a.K = c->K;
-    a.nf = c->nf;
-    a.dt = dt;
-    a.c = c->p.c;
-    a.w0 = w0;
-    a.w1 = w1;
-    a.inv_Pr = 1.0 / c->p.Pr;
-    a.Re_i = c->p.Re_i;
-    a.Re_o = c->p.Re_o;
     const int plane = c->M1 * c->NK;
-    dim3 gridp((plane + 127) / 128, c->N_r);
-    if (c->lin_fused) {
+    {
         FusedArgs fa{};
         for (int i = 0; i < c->nf; ++i) {
             fa.u[i] = c->state[i];
@@ -1176,29 +868,7 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
         k_poisson_bwd_correct<<<(plane + PBB - 1) / PBB, PBB, PIPE_PB * sizeof(PBwdSlot), c->stream>>>(pa);
         prof_end(c);
         NSC_CUDA(c, cudaGetLastError());
-        return NSC_OK;
     }
-    prof_begin(c, NSC_K_RHS);
-    k_rhs<<<gridp, 128, 0, c->stream>>>(a);
-    prof_end(c);
-    NSC_CUDA(c, cudaGetLastError());
-    if ((rc = run_solve(c, c->facH[0], c->shH, c->W[0], false))) return rc;
-    if ((rc = run_solve(c, c->facH[1], c->shH, c->W[1], false))) return rc;
-    if ((rc = run_solve(c, c->facH[2], c->shH, c->W[2], false))) return rc;
-    if (c->heated)
-        if ((rc = run_solve(c, c->facT_shared ? c->facH[2] : c->facH[3], c->shH, c->W[3], false))) return rc;
-    prof_begin(c, NSC_K_RECOMBINE);
-    k_recombine<<<(unsigned)((c->F + 255) / 256), 256, 0, c->stream>>>(a, c->F);
-    prof_end(c);
-    prof_begin(c, NSC_K_DIV);
-    k_div<<<gridp, 128, 0, c->stream>>>(a);
-    prof_end(c);
-    NSC_CUDA(c, cudaGetLastError());
-    if ((rc = run_solve(c, c->facP, c->shP, c->G, true))) return rc;
-    prof_begin(c, NSC_K_CORRECT);
-    k_correct<<<gridp, 128, 0, c->stream>>>(a);
-    prof_end(c);
-    NSC_CUDA(c, cudaGetLastError());
     return NSC_OK;
 }
 

@@ -74,7 +74,6 @@ struct nsc_ctx {
     bool facT_shared = false;             // T shares the u_z factors (Pr == 1)
     double fac_dt = 0.0;                  // dt the Helmholtz factors were built for (0: none)
     bool facP_ready = false;
-    bool lin_fused = true;                // fused sweeps k_rhs_fwd / k_bwd_div (NSC_LIN_VARIANT=0: separate kernels)
     bool have_state = false;
     std::string err;
     long long launches = 0;
