@@ -158,6 +158,24 @@ template <int NPEND> __device__ __forceinline__ void cpa_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(NPEND) : "memory");
 }
 
+// The substitution windows are rings indexed by (row & (ring - 1)) held in registers; the row loops are
+// unrolled by the ring length so that every ring index is a compile-time constant (no register moves).
+template <int R> struct RowTag { static constexpr int value = R; };
+#define NSC_ROWS8(F, j0)                                                                             \
+    F(RowTag<0>{}, (j0) + 0); F(RowTag<1>{}, (j0) + 1); F(RowTag<2>{}, (j0) + 2); F(RowTag<3>{}, (j0) + 3); \
+    F(RowTag<4>{}, (j0) + 4); F(RowTag<5>{}, (j0) + 5); F(RowTag<6>{}, (j0) + 6); F(RowTag<7>{}, (j0) + 7)
+#define NSC_ROWS16(F, j0) \
+    NSC_ROWS8(F, j0);     \
+    F(RowTag<8>{}, (j0) + 8); F(RowTag<9>{}, (j0) + 9); F(RowTag<10>{}, (j0) + 10); F(RowTag<11>{}, (j0) + 11); \
+    F(RowTag<12>{}, (j0) + 12); F(RowTag<13>{}, (j0) + 13); F(RowTag<14>{}, (j0) + 14); F(RowTag<15>{}, (j0) + 15)
+#define NSC_ROWS16_DOWN(F, j0) \
+    F(RowTag<15>{}, (j0) + 15); F(RowTag<14>{}, (j0) + 14); F(RowTag<13>{}, (j0) + 13); F(RowTag<12>{}, (j0) + 12); \
+    F(RowTag<11>{}, (j0) + 11); F(RowTag<10>{}, (j0) + 10); F(RowTag<9>{}, (j0) + 9); F(RowTag<8>{}, (j0) + 8); \
+    NSC_ROWS8_DOWN(F, j0)
+#define NSC_ROWS8_DOWN(F, j0)                                                                        \
+    F(RowTag<7>{}, (j0) + 7); F(RowTag<6>{}, (j0) + 6); F(RowTag<5>{}, (j0) + 5); F(RowTag<4>{}, (j0) + 4); \
+    F(RowTag<3>{}, (j0) + 3); F(RowTag<2>{}, (j0) + 2); F(RowTag<1>{}, (j0) + 1); F(RowTag<0>{}, (j0) + 0)
+
 // k_rhs_fwd: block = (PBK modes) x (NF fields).  Slot arrays: u[NF], p, DP, E0[NF], E1[NF] (if present).
 template <int NF> struct FwdSlot {
     cd fld[3 * NF + 2][PBK];
@@ -209,12 +227,14 @@ __global__ void __launch_bounds__(PBK * NF) k_rhs_fwd(FusedArgs a) {
         }
         cpa_commit();
     };
-    cd w[FW];                                           // w[FW-1] = most recent row
+    cd w[FW];                                           // ring: y_j lives in w[j & 7]
 #pragma unroll
     for (int i = 0; i < FW; ++i) w[i] = mk(0.0, 0.0);
 #pragma unroll
     for (int d = 0; d < PIPE_F - 1; ++d) issue(d);
-    for (int j = 0; j < N; ++j) {
+    auto row = [&](auto tag, int j) {
+        constexpr int R = decltype(tag)::value;
+        if (j >= N) return;
         cpa_wait<PIPE_F - 2>();
         __syncthreads();
         issue(j + PIPE_F - 1);
@@ -255,31 +275,31 @@ __global__ void __launch_bounds__(PBK * NF) k_rhs_fwd(FusedArgs a) {
                 b = mk(fma(dt, E.x, ic * u.x), fma(dt, E.y, ic * u.y));
             }
         }
-        // forward substitution: y_j = b_j - sum_i L[j][i] y_{lo + i}
+        // forward substitution: y_j = b_j - sum_{d=1..nl} L[j][nl - d] y_{j-d}
         if (j >= ja && j < jb) {
 #pragma unroll
-            for (int i = 0; i < FWI; ++i) {
-                const double l = s.L[fld][i][tx];
-                b.x = fma(-l, w[FW - FWI + i].x, b.x);
-                b.y = fma(-l, w[FW - FWI + i].y, b.y);
+            for (int d = FWI; d >= 1; --d) {
+                const double l = s.L[fld][FWI - d][tx];
+                b.x = fma(-l, w[(R - d) & 7].x, b.x);
+                b.y = fma(-l, w[(R - d) & 7].y, b.y);
             }
         } else {
             const int nl = j - a.lo[j];
             const double* Lr = Lf + (size_t)a.offL[j] * P;
 #pragma unroll
-            for (int q = 0; q < FW; ++q) {
-                const int i = q - (FW - nl);
-                if (i >= 0) {
-                    const double l = Lr[(size_t)i * P];
-                    b.x = fma(-l, w[q].x, b.x);
-                    b.y = fma(-l, w[q].y, b.y);
+            for (int d = FW - 1; d >= 1; --d) {
+                if (d <= nl) {
+                    const double l = Lr[(size_t)(nl - d) * P];
+                    b.x = fma(-l, w[(R - d) & 7].x, b.x);
+                    b.y = fma(-l, w[(R - d) & 7].y, b.y);
                 }
             }
         }
-#pragma unroll
-        for (int q = 0; q < FW - 1; ++q) w[q] = w[q + 1];
-        w[FW - 1] = b;
+        w[R] = b;
         if (valid) Wf[(size_t)j * plane + e] = b;
+    };
+    for (int j0 = 0; j0 < N; j0 += 8) {
+        NSC_ROWS8(row, j0);
     }
     cpa_wait<0>();
 }
@@ -339,7 +359,7 @@ __global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
         }
         cpa_commit();
     };
-    cd w[FW];                                           // back-substitution window, w[0] = x_{j+1}
+    cd w[FW];                                           // back-substitution ring: x_j lives in w[j & 7]
 #pragma unroll
     for (int i = 0; i < FW; ++i) w[i] = mk(0.0, 0.0);
     // divergence role, row j (its x_+, x_-, x_z were left in exch[j & 1] one iteration earlier)
@@ -379,7 +399,9 @@ __global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
     };
 #pragma unroll
     for (int d = 0; d < PIPE_B - 1; ++d) issue(N - 1 - d);
-    for (int j = N - 1; j >= 0; --j) {
+    auto row = [&](auto tag, int j) {
+        constexpr int R = decltype(tag)::value;
+        if (j >= N) return;
         cpa_wait<PIPE_B - 2>();
         __syncthreads();                                 // row j has arrived; exch[(j + 1) & 1] is complete
         issue(j - (PIPE_B - 1));
@@ -387,30 +409,29 @@ __global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
         const size_t o = (size_t)j * plane + e;
         if (is_field) {
             cd y = s.fld[f][tx];
+            // x_j = (y_j - sum_{d=1..nu} U[j][d] x_{j+d}) / pivot;  x_j lives in w[j & 7]
             if (j >= ja && j < jb) {
 #pragma unroll
-                for (int q = 0; q < FWI; ++q) {
-                    const double u = s.U[f][q + 1][tx];
-                    y.x = fma(-u, w[q].x, y.x);
-                    y.y = fma(-u, w[q].y, y.y);
+                for (int d = FWI; d >= 1; --d) {
+                    const double u = s.U[f][d][tx];
+                    y.x = fma(-u, w[(R + d) & 7].x, y.x);
+                    y.y = fma(-u, w[(R + d) & 7].y, y.y);
                 }
                 y = s.U[f][0][tx] * y;
             } else {
                 const int nu = a.hi[j] - j;
                 const double* Ur = Uf + (size_t)a.offU[j] * P;
 #pragma unroll
-                for (int q = 0; q < FW; ++q) {
-                    if (q < nu) {
-                        const double u = Ur[(size_t)(q + 1) * P];
-                        y.x = fma(-u, w[q].x, y.x);
-                        y.y = fma(-u, w[q].y, y.y);
+                for (int d = FW - 1; d >= 1; --d) {
+                    if (d <= nu) {
+                        const double u = Ur[(size_t)d * P];
+                        y.x = fma(-u, w[(R + d) & 7].x, y.x);
+                        y.y = fma(-u, w[(R + d) & 7].y, y.y);
                     }
                 }
                 y = Ur[0] * y;
             }
-#pragma unroll
-            for (int q = FW - 1; q > 0; --q) w[q] = w[q - 1];
-            w[0] = y;
+            w[R] = y;
             cd u;                                        // u_f of the state the sub-step starts from
             if (f < 2) {
                 const cd ur = s.fld[NF][tx], ut = s.fld[NF + 1][tx];
@@ -423,6 +444,9 @@ __global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
             if (f >= 2 && valid) Wf[o] = x;
         }
         if (!is_field && j < N - 1) div_row(j + 1);      // one row behind the field roles
+    };
+    for (int j0 = (N - 1) & ~7; j0 >= 0; j0 -= 8) {
+        NSC_ROWS8_DOWN(row, j0);
     }
     __syncthreads();
     if (!is_field) div_row(0);
@@ -456,7 +480,7 @@ struct PoisArgs {
 
 constexpr int PBP = 128;    // modes per block, forward sweep
 constexpr int PBB = 64;     // modes per block, backward sweep + correction
-constexpr int PW = 12;      // substitution window (Poisson envelope <= 12)
+constexpr int PW = 16;      // substitution ring (Poisson envelope <= 12)
 constexpr int PWI = 8;      // interior lower / upper width
 
 struct PFwdSlot {
@@ -490,41 +514,44 @@ __global__ void __launch_bounds__(PBP) k_poisson_fwd(PoisArgs a) {
         }
         cpa_commit();
     };
-    cd w[PW];                                           // w[PW-1] = most recent row
+    cd w[PW];                                           // ring: y_j lives in w[j & 15]
 #pragma unroll
     for (int i = 0; i < PW; ++i) w[i] = mk(0.0, 0.0);
 #pragma unroll
     for (int d = 0; d < PIPE_PF - 1; ++d) issue(d);
-    for (int j = 0; j < N; ++j) {
+    auto row = [&](auto tag, int j) {
+        constexpr int R = decltype(tag)::value;
+        if (j >= N) return;
         cpa_wait<PIPE_PF - 2>();
         __syncthreads();
         issue(j + PIPE_PF - 1);
         const PFwdSlot& s = slots[j % PIPE_PF];
         cd b = s.g[tx];
+        // y_j = b_j - sum_{d=1..nl} L[j][nl - d] y_{j-d}
         if (j >= a.jaL && j < a.jbL) {
 #pragma unroll
-            for (int i = 0; i < PWI; ++i) {
-                const double l = s.L[i][tx];
-                b.x = fma(-l, w[PW - PWI + i].x, b.x);
-                b.y = fma(-l, w[PW - PWI + i].y, b.y);
+            for (int d = PWI; d >= 1; --d) {
+                const double l = s.L[PWI - d][tx];
+                b.x = fma(-l, w[(R - d) & 15].x, b.x);
+                b.y = fma(-l, w[(R - d) & 15].y, b.y);
             }
         } else {
             const int nl = j - a.lo[j];
             const double* Lr = Lf + (size_t)a.offL[j] * P;
 #pragma unroll
-            for (int q = 0; q < PW; ++q) {
-                const int i = q - (PW - nl);
-                if (i >= 0) {
-                    const double l = Lr[(size_t)i * P];
-                    b.x = fma(-l, w[q].x, b.x);
-                    b.y = fma(-l, w[q].y, b.y);
+            for (int d = 12; d >= 1; --d) {
+                if (d <= nl) {
+                    const double l = Lr[(size_t)(nl - d) * P];
+                    b.x = fma(-l, w[(R - d) & 15].x, b.x);
+                    b.y = fma(-l, w[(R - d) & 15].y, b.y);
                 }
             }
         }
-#pragma unroll
-        for (int q = 0; q < PW - 1; ++q) w[q] = w[q + 1];
-        w[PW - 1] = b;
+        w[R] = b;
         if (valid) a.G[(size_t)j * plane + e] = b;
+    };
+    for (int j0 = 0; j0 < N; j0 += 16) {
+        NSC_ROWS16(row, j0);
     }
     cpa_wait<0>();
 }
@@ -539,7 +566,6 @@ struct PBwdSlot {
 __global__ void __launch_bounds__(PBB) k_poisson_bwd_correct(PoisArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PBwdSlot* slots = reinterpret_cast<PBwdSlot*>(smem_raw);
-    __shared__ cd ring[16][PBB];                        // phi of the last rows; column tx is private to thread tx
     const int tx = threadIdx.x;
     const int plane_i = a.M1 * a.NK;
     const int e0 = blockIdx.x * PBB + tx;
@@ -580,44 +606,9 @@ __global__ void __launch_bounds__(PBB) k_poisson_bwd_correct(PoisArgs a) {
         }
         cpa_commit();
     };
-    // L5 at row jc from (u_r*, u_theta*, u_z*, T, p, D1 p) of that row
-    auto correct = [&](int jc, cd ur, cd ut, cd uz, cd T, cd pr, cd dp) {
-        const size_t oc = (size_t)jc * plane + e;
-        const cd phi = ring[jc & 15][tx];
-        cd gphi = mk(0.0, 0.0);
-        if (jc != 0 && jc != N - 1) {
-            const int s0 = a.s0[jc];
-            const double* d = a.D1 + jc * NPT;
+    cd w[12];                                           // w[d] = phi_{j+d}, d = 0 .. 11 (shifted every row)
 #pragma unroll
-            for (int l = 0; l < NPT; ++l) {
-                const double wt = __ldg(d + l);
-                const cd v = ring[(s0 + l) & 15][tx];
-                gphi.x = fma(wt, v.x, gphi.x);
-                gphi.y = fma(wt, v.y, gphi.y);
-            }
-        }
-        if (!valid) return;
-        const double nr = n * a.rinv[jc];
-        cd o0 = ur - gphi;
-        if (m00) o0 = mk(0.0, 0.0);
-        a.dst[0][oc] = o0;
-        a.dst[1][oc] = mk(ut.x + nr * phi.y, ut.y - nr * phi.x);          // - (i n / r) phi
-        a.dst[2][oc] = mk(uz.x + kap * phi.y, uz.y - kap * phi.x);        // - i kappa phi
-        if (a.copyT) a.dst[3][oc] = T;
-        if (have_p) {
-            a.p_dst[oc] = mk(fma(idt, phi.x, pr.x), fma(idt, phi.y, pr.y));
-            a.DP[oc] = mk(fma(idt, gphi.x, dp.x), fma(idt, gphi.y, dp.y));
-        }
-    };
-    auto correct_direct = [&](int jc) {                  // rows next to the walls: operands straight from HBM
-        const size_t oc = (size_t)jc * plane + e;
-        const cd z = mk(0.0, 0.0);
-        correct(jc, a.W[0][oc], a.W[1][oc], a.W[2][oc], a.copyT ? a.W[3][oc] : z, have_p ? a.p[oc] : z,
-                have_p ? a.DP[oc] : z);
-    };
-    cd w[PW];                                           // w[0] = phi_{j+1}
-#pragma unroll
-    for (int i = 0; i < PW; ++i) w[i] = mk(0.0, 0.0);
+    for (int i = 0; i < 12; ++i) w[i] = mk(0.0, 0.0);
 #pragma unroll
     for (int d = 0; d < PIPE_PB - 1; ++d) issue(N - 1 - d);
     for (int j = N - 1; j >= 0; --j) {
@@ -626,40 +617,83 @@ __global__ void __launch_bounds__(PBB) k_poisson_bwd_correct(PoisArgs a) {
         issue(j - (PIPE_PB - 1));
         const PBwdSlot& s = slots[(N - 1 - j) % PIPE_PB];
         cd y = s.y[tx];
+        // phi_j = (y_j - sum_{d=1..nu} U[j][d] phi_{j+d}) / pivot;  here w[d-1] = phi_{j+d}
         if (j >= a.jaU && j < a.jbU) {
 #pragma unroll
-            for (int q = 0; q < PWI; ++q) {
-                const double u = s.U[q + 1][tx];
-                y.x = fma(-u, w[q].x, y.x);
-                y.y = fma(-u, w[q].y, y.y);
+            for (int d = PWI; d >= 1; --d) {
+                const double u = s.U[d][tx];
+                y.x = fma(-u, w[d - 1].x, y.x);
+                y.y = fma(-u, w[d - 1].y, y.y);
             }
             y = s.U[0][tx] * y;
         } else {
             const int nu = a.hi[j] - j;
             const double* Ur = Uf + (size_t)a.offU[j] * P;
 #pragma unroll
-            for (int q = 0; q < PW; ++q) {
-                if (q < nu) {
-                    const double u = Ur[(size_t)(q + 1) * P];
-                    y.x = fma(-u, w[q].x, y.x);
-                    y.y = fma(-u, w[q].y, y.y);
+            for (int d = 12; d >= 1; --d) {
+                if (d <= nu) {
+                    const double u = Ur[(size_t)d * P];
+                    y.x = fma(-u, w[d - 1].x, y.x);
+                    y.y = fma(-u, w[d - 1].y, y.y);
                 }
             }
             y = Ur[0] * y;
         }
 #pragma unroll
-        for (int q = PW - 1; q > 0; --q) w[q] = w[q - 1];
+        for (int q = 11; q > 0; --q) w[q] = w[q - 1];
         w[0] = y;
-        ring[j & 15][tx] = y;
-        if (j == N - 1) correct_direct(N - 1);
-        if (j <= N - NPT) {
-            if (j == N - NPT)
-                for (int jc = N - 2; jc > j + NPT / 2; --jc) correct_direct(jc);
+        // L5 at the rows jc whose stencil rows j .. j + 8 = w[0 .. 8] are now complete (wall rows: no stencil);
+        // the regular row jc = j + 4 has its operands in the slot, rows next to the walls read them from HBM
+        int c_hi = -1, c_lo = 0;
+        if (j == N - 1) {
+            c_hi = c_lo = N - 1;
+        } else if (j <= N - NPT) {
+            c_hi = (j == N - NPT) ? N - 2 : j + NPT / 2;
+            c_lo = (j == 0) ? 0 : j + NPT / 2;
+        }
+        for (int jc = c_hi; jc >= c_lo; --jc) {
+            const size_t oc = (size_t)jc * plane + e;
+            const bool piped = (jc == j + NPT / 2) && (j <= N - NPT);
             const cd z = mk(0.0, 0.0);
-            correct(j + NPT / 2, s.op[0][tx], s.op[1][tx], s.op[2][tx], a.copyT ? s.op[3][tx] : z,
-                    have_p ? s.op[MAXF][tx] : z, have_p ? s.op[MAXF + 1][tx] : z);
-            if (j == 0)
-                for (int jc = NPT / 2 - 1; jc >= 0; --jc) correct_direct(jc);
+            const cd ur = piped ? s.op[0][tx] : a.W[0][oc];
+            const cd ut = piped ? s.op[1][tx] : a.W[1][oc];
+            const cd uz = piped ? s.op[2][tx] : a.W[2][oc];
+            const cd T = a.copyT ? (piped ? s.op[3][tx] : a.W[3][oc]) : z;
+            const cd pr = have_p ? (piped ? s.op[MAXF][tx] : a.p[oc]) : z;
+            const cd dp = have_p ? (piped ? s.op[MAXF + 1][tx] : a.DP[oc]) : z;
+            cd phi = w[NPT / 2];
+            if (!piped) {                                // phi_jc = w[jc - j], picked by an exact 0/1 blend (keeps w in registers)
+                phi = mk(0.0, 0.0);
+#pragma unroll
+                for (int d = 0; d < NPT; ++d) {
+                    const double sel = (d == jc - j) ? 1.0 : 0.0;
+                    phi.x = fma(sel, w[d].x, phi.x);
+                    phi.y = fma(sel, w[d].y, phi.y);
+                }
+            }
+            cd gphi = mk(0.0, 0.0);
+            if (jc != 0 && jc != N - 1) {
+                const double* dd = a.D1 + jc * NPT;
+#pragma unroll
+                for (int l = 0; l < NPT; ++l) {
+                    const double wt = __ldg(dd + l);
+                    gphi.x = fma(wt, w[l].x, gphi.x);
+                    gphi.y = fma(wt, w[l].y, gphi.y);
+                }
+            }
+            if (valid) {
+                const double nr = n * a.rinv[jc];
+                cd o0 = ur - gphi;
+                if (m00) o0 = mk(0.0, 0.0);
+                a.dst[0][oc] = o0;
+                a.dst[1][oc] = mk(ut.x + nr * phi.y, ut.y - nr * phi.x);          // - (i n / r) phi
+                a.dst[2][oc] = mk(uz.x + kap * phi.y, uz.y - kap * phi.x);        // - i kappa phi
+                if (a.copyT) a.dst[3][oc] = T;
+                if (have_p) {
+                    a.p_dst[oc] = mk(fma(idt, phi.x, pr.x), fma(idt, phi.y, pr.y));
+                    a.DP[oc] = mk(fma(idt, gphi.x, dp.x), fma(idt, gphi.y, dp.y));
+                }
+            }
         }
     }
     cpa_wait<0>();
