@@ -24,8 +24,8 @@ template <class Kern> static int set_smem(Kern k, size_t smem, bool& done) {
 }
 
 int launch_dr(const DrArgs& a, int nf, cudaStream_t st) {
-    dim3 grid((unsigned)((a.plane + 127) / 128), nf);
-    k_dr<<<grid, 128, 0, st>>>(a);
+    dim3 grid((unsigned)((a.plane + DR_TB - 1) / DR_TB), nf);
+    k_dr<<<grid, DR_TB, 0, st>>>(a);
     return (int)cudaGetLastError();
 }
 

@@ -26,33 +26,50 @@ namespace nsc {
 
 // ------------------------------------------------------------------------------------------ k_dr
 // out[j] = sum_l D1[j][l] f[s0(j) + l],  s0(j) = clamp(j - 4, 0, N_r - 9)   (O2, R3)
-constexpr int DR_LA = 3;   // levels loaded ahead of the window (memory-level parallelism)
-__global__ void __launch_bounds__(128) k_dr(DrArgs a) {
-    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (col >= a.plane) return;
+// One thread per (mode, field) marches over j; the rows of f arrive by cp.async in a 16-row
+// shared-memory ring up to seven rows ahead of the stencil (column threadIdx.x of the ring is private).
+constexpr int DR_TB = 128;  // modes per block
+constexpr int DR_PRE = 12;  // rows requested up front; row j + DR_PRE is requested after row j is done, so the
+                            // ring holds rows j - 3 .. j + 12 (16 rows) when row j + 1 starts
+__global__ void __launch_bounds__(DR_TB) k_dr(DrArgs a) {
+    __shared__ __align__(16) cd ring[16][DR_TB];
+    const int tx = threadIdx.x;
+    const size_t col0 = (size_t)blockIdx.x * DR_TB + tx;
+    const bool valid = col0 < a.plane;
+    const size_t col = valid ? col0 : a.plane - 1;
     const cd* src = a.f[blockIdx.y] + col;
     cd* dst = a.out[blockIdx.y] + col;
     const int N = a.N_r;
-    cd w[NPT + DR_LA];
-#pragma unroll
-    for (int l = 0; l < NPT + DR_LA; ++l) w[l] = (l < N) ? src[(size_t)l * a.plane] : mk(0.0, 0.0);
-    for (int j = 0; j < N; ++j) {
-        if (j > NPT / 2 && j <= N - 1 - NPT / 2) {   // the window start advanced by one level
-#pragma unroll
-            for (int l = 0; l < NPT + DR_LA - 1; ++l) w[l] = w[l + 1];
-            const int nxt = j - NPT / 2 + NPT - 1 + DR_LA;
-            w[NPT + DR_LA - 1] = (nxt < N) ? src[(size_t)nxt * a.plane] : mk(0.0, 0.0);
+    auto issue = [&](int row) {
+        if (row < N) {
+            const uint32_t d = (uint32_t)__cvta_generic_to_shared(&ring[row & 15][tx]);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src + (size_t)row * a.plane) : "memory");
         }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+#pragma unroll
+    for (int r = 0; r < DR_PRE; ++r) issue(r);
+    for (int j = 0; j < N; ++j) {
+        // groups committed so far: rows 0 .. DR_PRE - 1 + j; rows 0 .. max(8, j + 4) must be complete
+        if (j <= NPT / 2) {
+            asm volatile("cp.async.wait_group %0;" ::"n"(DR_PRE - NPT) : "memory");
+        } else {
+            asm volatile("cp.async.wait_group %0;" ::"n"(DR_PRE - 1 - NPT / 2) : "memory");
+        }
+        const int s0 = j < NPT / 2 ? 0 : (j > N - 1 - NPT / 2 ? N - NPT : j - NPT / 2);
         const double* d = a.D1 + j * NPT;
         cd acc = mk(0.0, 0.0);
 #pragma unroll
         for (int l = 0; l < NPT; ++l) {
             const double c = __ldg(d + l);
-            acc.x = fma(c, w[l].x, acc.x);
-            acc.y = fma(c, w[l].y, acc.y);
+            const cd v = ring[(s0 + l) & 15][tx];
+            acc.x = fma(c, v.x, acc.x);
+            acc.y = fma(c, v.y, acc.y);
         }
-        dst[(size_t)j * a.plane] = acc;
+        if (valid) dst[(size_t)j * a.plane] = acc;
+        issue(DR_PRE + j);
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
 // ------------------------------------------------------------------------------------------
