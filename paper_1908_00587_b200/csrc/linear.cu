@@ -214,11 +214,18 @@ __global__ void __launch_bounds__(PBK * NF) k_rhs_fwd(FusedArgs a) {
         q -= NF;
         return q == 0 ? a.E1[0] : q == 1 ? a.E1[1] : q == 2 ? a.E1[2] : a.E1[3];
     };
+    // this thread requests arrays fld, fld + NF, ... of every row: source pointers resolved once
+    constexpr int NQ = (3 * NF + 2 + NF - 1) / NF;
+    const cd* gp[NQ];
+#pragma unroll
+    for (int k = 0; k < NQ; ++k) gp[k] = (fld + k * NF < narr) ? src_of(fld + k * NF) + e : nullptr;
     auto issue = [&](int j) {
         if (j < N) {
             FwdSlot<NF>& s = slots[j % PIPE_F];
-            const size_t o = (size_t)j * plane + e;
-            for (int q = fld; q < narr; q += NF) cpa16(&s.fld[q][tx], src_of(q) + o);
+            const size_t o = (size_t)j * plane;
+#pragma unroll
+            for (int k = 0; k < NQ; ++k)
+                if (gp[k]) cpa16(&s.fld[fld + k * NF][tx], gp[k] + o);
             if (j >= ja && j < jb) {
                 const double* Lr = Lf + (size_t)(a.offL4 + FWI * (j - ja)) * P;
 #pragma unroll
@@ -345,12 +352,19 @@ __global__ void __launch_bounds__(PBK * (NF + 1)) k_bwd_div(FusedArgs a) {
         q -= NF;
         return q == 0 ? a.u[0] : q == 1 ? a.u[1] : q == 2 ? a.u[2] : a.u[3];
     };
+    // this thread requests arrays role, role + NF + 1 of every row: source pointers resolved once
+    constexpr int NQ = (2 * NF + NF) / (NF + 1);
+    const cd* gp[NQ];
+#pragma unroll
+    for (int k = 0; k < NQ; ++k) gp[k] = (role + k * (NF + 1) < 2 * NF) ? src_of(role + k * (NF + 1)) + e : nullptr;
     // row j travels in slot (N - 1 - j) % PIPE_B
     auto issue = [&](int j) {
         if (j >= 0) {
             BwdSlot<NF>& s = slots[(N - 1 - j) % PIPE_B];
-            const size_t o = (size_t)j * plane + e;
-            for (int q = role; q < 2 * NF; q += NF + 1) cpa16(&s.fld[q][tx], src_of(q) + o);
+            const size_t o = (size_t)j * plane;
+#pragma unroll
+            for (int k = 0; k < NQ; ++k)
+                if (gp[k]) cpa16(&s.fld[role + k * (NF + 1)][tx], gp[k] + o);
             if (is_field && j >= ja && j < jb) {
                 const double* Ur = Uf + (size_t)(a.offU4 + (FWI + 1) * (j - ja)) * P;
 #pragma unroll
