@@ -255,7 +255,7 @@ def workload_name(cfg):
 
 def run_ours(args, cfg, rank, world, local_rank):
     import torch
-    from paper_1908_00587_b200 import build, nsc, synth
+    from paper_1908_00587_b200 import build, nsc, synth, replicas
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local_rank)
@@ -280,7 +280,7 @@ def run_ours(args, cfg, rank, world, local_rank):
 
     with nsc.Context.from_config(cfg, radial_chunk=args.radial_chunk) as ctx:
         ctx.set_stream(stream)
-        st = synth.make_state(dict(cfg, seed=cfg["seed"] + 1000 * rank), ctx.grid())
+        st = synth.make_state(replicas.rank_config(cfg, rank), ctx.grid())
         # pinned host copies of the state (inputs of a step) and of the result
         names = [0, 1, 2] + ([3] if nf == 4 else []) + [4]
         pin_in, pin_out = {}, {}
@@ -311,10 +311,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         ms = ev0.elapsed_time(ev1)
         launches = ctx.launch_count() - l0
         clk = clocks.stop() if rank == 0 else None
-        if dist is not None:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = replicas.max_over_ranks(ms, dist, "cuda")
         ms_per_step = ms / args.steps
 
         # ---- per-kernel CUDA-event timing of the same K steps (events bracket every launch)
@@ -342,10 +339,7 @@ def run_ours(args, cfg, rank, world, local_rank):
             ctx.get_state(*host_out)          # nsc_get_state_host: device -> pinned host, synchronises
         torch.cuda.synchronize()
         e2e_s = (time.perf_counter() - t0) / ke
-        if dist is not None:
-            t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = replicas.max_over_ranks(e2e_s, dist, "cuda")
         finite = bool(np.isfinite(host_out[1]).all())
         dev_bytes = ctx.device_bytes()
 
@@ -406,7 +400,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         "kernels": kern + [lin],
         "ms_per_step_with_event_brackets": ms_prof_per_step,
     }
-    value = world * args.steps / (ms / 1e3)
+    value = replicas.aggregate_rate(world, args.steps, ms / 1e3)
     mode_points = s["N_r"] * (s["M"] + 1) * (2 * s["K"] + 1)
     nbytes_state = len(names) * F
     out = {
@@ -421,7 +415,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         "mode_points_per_s": value * mode_points,
         "gpu_launches": launches,
         "clocks": clk,
-        "e2e": {"value": world / e2e_s, "unit": "steps/s", "h2d_bytes_per_step": nbytes_state,
+        "e2e": {"value": replicas.aggregate_rate(world, 1, e2e_s), "unit": "steps/s", "h2d_bytes_per_step": nbytes_state,
                 "d2h_bytes_per_step": nbytes_state, "steps": ke,
                 "what": "nsc_set_state_host (pinned) + nsc_step + nsc_get_state_host per step"},
         "roofline": roofline,
