@@ -218,3 +218,24 @@ def test_full_size_cfg4_sampled(torch_cuda):
         # SURVEY T5 quotes <= 1e-9 for single modes at N_r = 256; over all 3.3e7 interior mode-points of the
         # broadband state the maximum is a few 1e-9 (cond(P) ~ 1e13 on the Chebyshev grid): bar 1e-8
         assert np.max(np.abs(d[mask]) / scale[mask]) <= 1e-8
+
+
+@pytest.mark.parametrize("ci,N_r,M,K", [(3, 12, 256, 256), (2, 17, 8, 16)])
+def test_step_is_deterministic(torch_cuda, ci, N_r, M, K):
+    """Two contexts, same state, three steps each: bit-identical results (R15: one deterministic result per
+    input).  A shared-memory race in the transform tiles or in the cp.async row pipelines of the marching
+    sweeps would show up here as run-to-run differences; (3, 12, 256, 256) runs the length-768 kernels."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    res = []
+    for _ in range(2):
+        with _ctx(cfg) as ctx:
+            st = synth.make_state(cfg, ctx.grid())
+            ctx.set_state(*_dev(torch, st))
+            for _ in range(3):
+                ctx.step(cfg["dt"])
+            res.append(ctx.state_to_host())
+    for a, b in zip(*res):
+        if a is not None:
+            assert np.isfinite(a).all()
+            np.testing.assert_array_equal(a, b)
