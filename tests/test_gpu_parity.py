@@ -239,3 +239,33 @@ def test_step_is_deterministic(torch_cuda, ci, N_r, M, K):
         if a is not None:
             assert np.isfinite(a).all()
             np.testing.assert_array_equal(a, b)
+
+
+@pytest.mark.parametrize("grid,c", [(0, 0.5), (1, 0.7), (1, 1.0), (0, 0.3)])
+def test_substep_uniform_grid_and_other_implicitness(torch_cuda, grid, c):
+    """The rewrite of L1 as u/c - gamma A u for gamma = (1-c)/c != 1 and gamma = 0,
+    and the uniform radial grid (R2 type 0): one sub-step and two full steps against the oracle."""
+    torch = torch_cuda
+    cfg = dict(synth.scaled_config(2, N_r=20, M=4, K=8), grid=grid)
+    nf = nf_of(cfg)
+    o = oracle_of(cfg, c=c)
+    with _ctx(cfg, c=c) as ctx:
+        np.testing.assert_array_equal(ctx.grid(), o.r)
+        st = synth.make_state(cfg, ctx.grid())
+        rng = np.random.default_rng(4)
+        st[4] = 5.0 * (rng.standard_normal(st[0].shape) + 1j * rng.standard_normal(st[0].shape))
+        U = max(abs(cfg["Re_i"]), abs(cfg["Re_o"]))
+        E = [U * U * 0.1 * f for f in _random_fields(cfg, 9, nf)]
+        ctx.set_state(*_dev(torch, st))
+        ctx.substep(*_dev(torch, E), cfg["dt"])
+        got = ctx.state_to_host()
+        ref = o.substep(st, E, cfg["dt"])
+        assert rel_l2(got[:nf], ref[:nf]) <= 1e-11
+        ctx.set_state(*_dev(torch, st))
+        for _ in range(2):
+            ctx.step(cfg["dt"])
+        got = ctx.state_to_host()
+    ref = st
+    for _ in range(2):
+        ref = o.step(ref, cfg["dt"])
+    assert rel_l2(got[:nf], ref[:nf]) <= TOL_STEP
