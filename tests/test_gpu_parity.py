@@ -180,15 +180,18 @@ def test_host_buffer_entry_points_and_errors(torch_cuda):
         assert ctx.launch_count() > n0
 
 
-def test_full_size_cfg4_sampled(torch_cuda):
-    """BASELINE.json configs[3] at full size (N_r = 256, M = K = 256, 768 x 768 grid), in the launch
-    configuration bench.py times (length-768 transform pipeline + fused linear sweeps): the nonlinear
-    term at sampled radial nodes and one sub-step at sampled modes against the oracle, then the
-    divergence of the stepped state at round-off (a property that holds at any size)."""
+@pytest.mark.parametrize("ci", [3, 2])
+def test_full_size_sampled(torch_cuda, ci):
+    """BASELINE.json configs[3] (N_r = 256, M = K = 256, 768 x 768 grid: bench.py's workload, length-768
+    transform pipeline + fused linear sweeps) and configs[2] (heated, 128^3, generic transform kernels) at full
+    size: the nonlinear term at sampled radial nodes and one sub-step at sampled modes against the oracle, then
+    the divergence of the stepped state at round-off (a property that holds at any size)."""
     torch = torch_cuda
-    cfg = synth.config(3)
+    cfg = synth.config(ci)
+    nf = nf_of(cfg)
+    N_r = cfg["N_r"]
     o = oracle_of(cfg, dft="fft")
-    nodes = [0, 1, 4, 127, 200, 251, 254, 255]
+    nodes = [0, 1, 4, N_r // 2 - 1, (3 * N_r) // 4, N_r - 5, N_r - 2, N_r - 1]
     rng = np.random.default_rng(11)
     im = np.concatenate([[0, 0, 0, cfg["M"], cfg["M"], 1], rng.integers(0, cfg["M"] + 1, 26)])
     ik = np.concatenate([[cfg["K"], cfg["K"] + 1, 0, 0, 2 * cfg["K"], cfg["K"] - 1], rng.integers(0, 2 * cfg["K"] + 1, 26)])
@@ -196,22 +199,22 @@ def test_full_size_cfg4_sampled(torch_cuda):
         st = synth.make_state(cfg, ctx.grid())
         ctx.set_state(*_dev(torch, st))
         got = ctx.nonlinear_to_host()
-        ref = o.nonlinear(*st[:3], nodes=nodes)
+        ref = o.nonlinear(*st[:nf], nodes=nodes)
         assert rel_l2([g[nodes] for g in got], ref) <= TOL_N
         # sub-step with the nonlinear term just computed as the explicit term
         E = got
-        ctx.substep(*_dev(torch, E), None, cfg["dt"])
+        ctx.substep(*(_dev(torch, E) + [None] * (4 - nf)), cfg["dt"])
         sub = ctx.state_to_host()
         ref_s = o.substep(st, E, cfg["dt"], modes=(im, ik))
-        got_s = [f[:, im, ik] for f in sub[:3]]
-        assert rel_l2(got_s, ref_s[:3]) <= TOL_STEP
+        got_s = [f[:, im, ik] for f in sub[:nf]]
+        assert rel_l2(got_s, ref_s[:nf]) <= TOL_STEP
         # scaled divergence of the new state (formula of SURVEY.md section 8(c), pin T5)
         ur, ut, uz = sub[:3]
         r = o.r[:, None, None]
         n = o.n[None, :, None]
         kap = o.kappa[None, None, :]
         d = o.divergence(ur, ut, uz)[1:-1]
-        scale = (np.abs(o.D1) @ np.abs(ur).reshape(cfg["N_r"], -1)).reshape(ur.shape) + np.abs(ur) / r \
+        scale = (np.abs(o.D1) @ np.abs(ur).reshape(N_r, -1)).reshape(ur.shape) + np.abs(ur) / r \
             + np.abs(n / r * ut) + np.abs(kap * uz)
         scale = scale[1:-1]
         mask = scale > 0
