@@ -123,8 +123,13 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
     c->F = (size_t)c->N_r * c->M1 * c->NK;
     c->P = c->M1 * (c->K + 1);
     // radial chunk of the transform pipeline: work arrays of ~2 GiB unless told otherwise
+    // default: the whole radius at once when the work arrays stay below an eighth of the device memory
+    // (cfg 4: 10 GB), else chunks of ~2 GiB
     const size_t per_level = (size_t)4 * c->nf * c->Nz * c->MP * sizeof(cd);
-    int jc = p.radial_chunk > 0 ? p.radial_chunk : (int)(((size_t)2 << 30) / per_level);
+    size_t mem_free = 0, mem_total = 0;
+    cudaMemGetInfo(&mem_free, &mem_total);
+    int jc = p.radial_chunk > 0 ? p.radial_chunk
+             : (per_level * (size_t)p.N_r <= mem_total / 8 ? p.N_r : (int)(((size_t)2 << 30) / per_level));
     if (jc < 1) jc = 1;
     if (jc > c->N_r) jc = c->N_r;
     c->JC = jc;
@@ -139,7 +144,7 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
         if (c->t768 > 2) c->t768 = 2;
     }
     int rc = build_plan(c);
-    if (!rc && c->z768)
+    if (!rc && c->z768 && c->JC < c->N_r)     // D1 f arrays of the multi-chunk transform pipeline
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->DR[i], c->F, false);
     if (!rc) {
         for (int i = 0; i < 5 && !rc; ++i)

@@ -66,8 +66,11 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
     a2.tw768 = c->t.tw768;
     a2.alpha = c->p.alpha;
     a2.ktheta0 = (double)c->p.k_theta0;
-    if (c->z768) {
-        // N1: D1 f of every field, once per evaluation (marching kernel)
+    // N1, radial derivative.  One radial chunk (JC = N_r): D1 is applied to the z-transformed fields inside the
+    // work array after k_zinv (two transforms per line instead of three; D1 commutes with the z transform).
+    // Several chunks: D1 f of every spectral field once per evaluation, transformed as a third line.
+    const bool dr_after_z = c->z768 && c->JC == c->N_r;
+    if (c->z768 && !dr_after_z) {
         DrArgs d{};
         for (int i = 0; i < c->nf; ++i) {
             d.f[i] = f[i];
@@ -94,6 +97,20 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
             return cuda_fail(c, (cudaError_t)e, "k_zinv launch");
         }
         prof_end(c);
+        if (dr_after_z) {
+            DrArgs d{};
+            const size_t qstride = (size_t)c->JC * c->Nz * c->MP;
+            for (int i = 0; i < c->nf; ++i) {
+                d.f[i] = c->zbuf + (size_t)(3 * i) * qstride;
+                d.out[i] = c->zbuf + (size_t)(3 * i + 2) * qstride;
+            }
+            d.D1 = c->t.D1;
+            d.N_r = c->N_r;
+            d.plane = (size_t)c->Nz * c->MP;
+            prof_begin(c, NSC_K_DR);
+            if (int e = launch_dr(d, c->nf, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_dr launch");
+            prof_end(c);
+        }
         a.tw = c->t.tw_t;
         prof_begin(c, NSC_K_THETA);
         if (c->t768) {

@@ -31,14 +31,22 @@ namespace nsc {
 constexpr int DR_TB = 128;  // modes per block
 constexpr int DR_PRE = 12;  // rows requested up front; row j + DR_PRE is requested after row j is done, so the
                             // ring holds rows j - 3 .. j + 12 (16 rows) when row j + 1 starts
+template <int R> struct DrRow { static constexpr int value = R; };
+#define NSC_DR_ROWS16(F, j0)                                                                              \
+    F(DrRow<0>{}, (j0) + 0); F(DrRow<1>{}, (j0) + 1); F(DrRow<2>{}, (j0) + 2); F(DrRow<3>{}, (j0) + 3);     \
+    F(DrRow<4>{}, (j0) + 4); F(DrRow<5>{}, (j0) + 5); F(DrRow<6>{}, (j0) + 6); F(DrRow<7>{}, (j0) + 7);     \
+    F(DrRow<8>{}, (j0) + 8); F(DrRow<9>{}, (j0) + 9); F(DrRow<10>{}, (j0) + 10); F(DrRow<11>{}, (j0) + 11); \
+    F(DrRow<12>{}, (j0) + 12); F(DrRow<13>{}, (j0) + 13); F(DrRow<14>{}, (j0) + 14); F(DrRow<15>{}, (j0) + 15)
+
 __global__ void __launch_bounds__(DR_TB) k_dr(DrArgs a) {
     __shared__ __align__(16) cd ring[16][DR_TB];
     const int tx = threadIdx.x;
     const size_t col0 = (size_t)blockIdx.x * DR_TB + tx;
     const bool valid = col0 < a.plane;
     const size_t col = valid ? col0 : a.plane - 1;
-    const cd* src = a.f[blockIdx.y] + col;
-    cd* dst = a.out[blockIdx.y] + col;
+    const int fi = blockIdx.y;
+    const cd* src = (fi == 0 ? a.f[0] : fi == 1 ? a.f[1] : fi == 2 ? a.f[2] : a.f[3]) + col;
+    cd* dst = (fi == 0 ? a.out[0] : fi == 1 ? a.out[1] : fi == 2 ? a.out[2] : a.out[3]) + col;
     const int N = a.N_r;
     auto issue = [&](int row) {
         if (row < N) {
@@ -49,25 +57,46 @@ __global__ void __launch_bounds__(DR_TB) k_dr(DrArgs a) {
     };
 #pragma unroll
     for (int r = 0; r < DR_PRE; ++r) issue(r);
-    for (int j = 0; j < N; ++j) {
-        // groups committed so far: rows 0 .. DR_PRE - 1 + j; rows 0 .. max(8, j + 4) must be complete
-        if (j <= NPT / 2) {
-            asm volatile("cp.async.wait_group %0;" ::"n"(DR_PRE - NPT) : "memory");
-        } else {
-            asm volatile("cp.async.wait_group %0;" ::"n"(DR_PRE - 1 - NPT / 2) : "memory");
-        }
-        const int s0 = j < NPT / 2 ? 0 : (j > N - 1 - NPT / 2 ? N - NPT : j - NPT / 2);
+    // register copy of the ring: row r lives in w[r & 15]; the march is unrolled by 16 so that every index is
+    // a compile-time constant; each row enters the registers once (one shared-memory read per result)
+    cd w[16];
+    asm volatile("cp.async.wait_group %0;" ::"n"(DR_PRE - NPT) : "memory");     // rows 0 .. 8
+#pragma unroll
+    for (int r = 0; r < NPT; ++r) w[r] = ring[r][tx];
+    auto row = [&](auto tag, int j) {
+        constexpr int R = decltype(tag)::value;
+        if (j >= N) return;
         const double* d = a.D1 + j * NPT;
         cd acc = mk(0.0, 0.0);
+        if (j > N - 1 - NPT / 2) {
+            // last rows: stencil rows N - 9 .. N - 1 (all loaded), ring position not static: from shared memory
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
 #pragma unroll
-        for (int l = 0; l < NPT; ++l) {
-            const double c = __ldg(d + l);
-            const cd v = ring[(s0 + l) & 15][tx];
-            acc.x = fma(c, v.x, acc.x);
-            acc.y = fma(c, v.y, acc.y);
+            for (int l = 0; l < NPT; ++l) {
+                const double c = __ldg(d + l);
+                const cd v = ring[(N - NPT + l) & 15][tx];
+                acc.x = fma(c, v.x, acc.x);
+                acc.y = fma(c, v.y, acc.y);
+            }
+        } else {
+            if (j > NPT / 2) {                          // row j + 4 enters the window
+                asm volatile("cp.async.wait_group %0;" ::"n"(DR_PRE - 1 - NPT / 2) : "memory");
+                w[(R + NPT / 2) & 15] = ring[(R + NPT / 2) & 15][tx];
+            }
+            // first rows (j <= 4): rows 0 .. 8 = w[0 .. 8]; interior: rows j - 4 .. j + 4
+#pragma unroll
+            for (int l = 0; l < NPT; ++l) {
+                const double c = __ldg(d + l);
+                const cd v = (R <= NPT / 2) ? ((j <= NPT / 2) ? w[l] : w[(R - NPT / 2 + l) & 15]) : w[(R - NPT / 2 + l) & 15];
+                acc.x = fma(c, v.x, acc.x);
+                acc.y = fma(c, v.y, acc.y);
+            }
         }
         if (valid) dst[(size_t)j * a.plane] = acc;
         issue(DR_PRE + j);
+    };
+    for (int j0 = 0; j0 < N; j0 += 16) {
+        NSC_DR_ROWS16(row, j0);
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
@@ -156,6 +185,9 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
         }
     };
     auto field_of = [&](int it) { return (it / mtiles) / a.nj; };
+    // without radial-derivative input (A.dr[0] null) only i kappa f and f are transformed: D1 is then
+    // applied to the z-transformed f by k_dr on the work array (D1 and the z transform commute)
+    const int ns = A.dr[0] ? 3 : 2;
     int item = blockIdx.x;
     if (item < A.nitems) fetch(a.f[field_of(item)], item);
     __syncthreads();                                    // twiddles
@@ -165,7 +197,7 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
         const int jl = r % a.nj, fi = r / a.nj;
         const bool vm = (mt * 4 + warp) < a.M1;
 #pragma unroll 1
-        for (int s = 0; s < 3; ++s) {
+        for (int s = 0; s < ns; ++s) {
             const int q = (s == 0) ? 1 : (s == 1 ? 0 : 2);
             cd x[32];
             if (s != 1) {
@@ -192,7 +224,7 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
             }
             if (s >= 1) {                               // the staged line is consumed: request the next one
                 __syncwarp();
-                if (s == 1) {
+                if (s == 1 && ns == 3) {
                     fetch(A.dr[fi], item);
                 } else {
                     const int nxt = item + gridDim.x;
