@@ -29,6 +29,7 @@ int launch_radial_derivative(nsc_ctx* c, const cd* f, cd* out) {
     d.D1 = c->t.D1;
     d.N_r = c->N_r;
     d.plane = (size_t)c->M1 * c->NK;
+    d.ncols = d.plane;
     prof_begin(c, NSC_K_DR);
     if (int e = launch_dr(d, 1, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_dr launch");
     prof_end(c);
@@ -80,6 +81,7 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
         d.D1 = c->t.D1;
         d.N_r = c->N_r;
         d.plane = (size_t)c->M1 * c->NK;
+        d.ncols = d.plane;
         prof_begin(c, NSC_K_DR);
         if (int e = launch_dr(d, c->nf, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_dr launch");
         prof_end(c);
@@ -99,14 +101,15 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
         prof_end(c);
         if (dr_after_z) {
             DrArgs d{};
-            const size_t qstride = (size_t)c->JC * c->Nz * c->MP;
+            const size_t qstride = (size_t)c->Nz * c->MP;
             for (int i = 0; i < c->nf; ++i) {
                 d.f[i] = c->zbuf + (size_t)(3 * i) * qstride;
                 d.out[i] = c->zbuf + (size_t)(3 * i + 2) * qstride;
             }
             d.D1 = c->t.D1;
             d.N_r = c->N_r;
-            d.plane = (size_t)c->Nz * c->MP;
+            d.plane = (size_t)3 * c->nf * qstride;
+            d.ncols = qstride;
             prof_begin(c, NSC_K_DR);
             if (int e = launch_dr(d, c->nf, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_dr launch");
             prof_end(c);

@@ -10,7 +10,7 @@
 //            registers and shared memory.
 //   k_zfwd   N6 forward z-FFT, truncation to |k| <= K, scaling 1/(N_theta N_z), buoyancy.
 //
-// Layout of the half-transformed work arrays: complex128 [q][JC][N_z][MP], MP = M+1 rounded up
+// Layout of the half-transformed work arrays: complex128 [j_local][q][N_z][MP] (the lines of one radial level are neighbours), MP = M+1 rounded up
 // to a multiple of 8, radial index local to the chunk.
 #pragma once
 #include "nsc_internal.h"
@@ -20,8 +20,8 @@ namespace nsc {
 struct NlArgs {
     const cd* f[MAXF];     // spectral input fields [N_r][M1][NK]
     cd* out[MAXF];         // spectral outputs N_r, N_theta, N_z, N_T
-    cd* zbuf;              // [3 nf][JC][Nz][MP]: q = 3 f + {0: f, 1: dz f, 2: dr f}
-    cd* tbuf;              // [nf][JC][Nz][MP]
+    cd* zbuf;              // [JC][3 nf][Nz][MP]: q = 3 f + {0: f, 1: dz f, 2: dr f}
+    cd* tbuf;              // [JC][nf][Nz][MP]
     const double* D1;
     const int* s0;
     const double* rinv;
@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(ZCfg<NZ>::THREADS) k_zinv(NlArgs a) {
     }
     fft_line<NZ, +1>(x, buf, tw, tau);
     {
-        cd* dst = a.zbuf + ((size_t)(3 * fi + 0) * a.JC + jl) * NZ * zstride + m;
+        cd* dst = a.zbuf + ((size_t)jl * 3 * a.nf + (3 * fi + 0)) * NZ * zstride + m;
         if (valid)
 #pragma unroll
             for (int e = 0; e < E; ++e) dst[(size_t)G::idx(e, tau) * zstride] = x[e];
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(ZCfg<NZ>::THREADS) k_zinv(NlArgs a) {
     }
     fft_line<NZ, +1>(x, buf, tw, tau);
     {
-        cd* dst = a.zbuf + ((size_t)(3 * fi + 1) * a.JC + jl) * NZ * zstride + m;
+        cd* dst = a.zbuf + ((size_t)jl * 3 * a.nf + (3 * fi + 1)) * NZ * zstride + m;
         if (valid)
 #pragma unroll
             for (int e = 0; e < E; ++e) dst[(size_t)G::idx(e, tau) * zstride] = x[e];
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(ZCfg<NZ>::THREADS) k_zinv(NlArgs a) {
     }
     fft_line<NZ, +1>(x, buf, tw, tau);
     {
-        cd* dst = a.zbuf + ((size_t)(3 * fi + 2) * a.JC + jl) * NZ * zstride + m;
+        cd* dst = a.zbuf + ((size_t)jl * 3 * a.nf + (3 * fi + 2)) * NZ * zstride + m;
         if (valid)
 #pragma unroll
             for (int e = 0; e < E; ++e) dst[(size_t)G::idx(e, tau) * zstride] = x[e];
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(ZCfg<NZ>::THREADS) k_zfwd(NlArgs a) {
     const int jl = line / a.M1, m = line % a.M1, j = a.j0 + jl;
     const int fi = blockIdx.y;
     const size_t zstride = a.MP;
-    const cd* src = a.tbuf + ((size_t)fi * a.JC + jl) * NZ * zstride + m;
+    const cd* src = a.tbuf + ((size_t)jl * a.nf + fi) * NZ * zstride + m;
     cd x[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) x[e] = src[(size_t)G::idx(e, tau) * zstride];
@@ -264,14 +264,15 @@ __global__ void __launch_bounds__(TCfg<NT>::THREADS) k_theta(NlArgs a) {
     if (!valid) line = nlines - 1;
     const int jl = line / a.Nz, z = line % a.Nz;
     const double ri = a.rinv[a.j0 + jl];
-    const size_t qstride = (size_t)a.JC * a.Nz * a.MP;
-    const size_t loff = ((size_t)jl * a.Nz + z) * a.MP;
+    const size_t qstride = (size_t)a.Nz * a.MP;
+    const size_t loff = ((size_t)jl * 3 * a.nf * a.Nz + z) * a.MP;       // line (j, z) of q = 0 in zbuf
+    const size_t loff_t = ((size_t)jl * a.nf * a.Nz + z) * a.MP;          // ... in tbuf
     const int M = a.M;
     // A_f = plain, B_f = d/dz, C_f = d/dr half-transformed lines of field f at this (j, z)
 #define LINE_A(f) (a.zbuf + (size_t)(3 * (f) + 0) * qstride + loff)
 #define LINE_B(f) (a.zbuf + (size_t)(3 * (f) + 1) * qstride + loff)
 #define LINE_C(f) (a.zbuf + (size_t)(3 * (f) + 2) * qstride + loff)
-#define LINE_O(f) (a.tbuf + (size_t)(f) * qstride + loff)
+#define LINE_O(f) (a.tbuf + (size_t)(f) * qstride + loff_t)
 #define UB(c, e) Ub[((c) * E + (e)) * TPL + tau]
     cd x[E];
     double acc0[E], acc1[E];

@@ -24,7 +24,7 @@ template <class Kern> static int set_smem(Kern k, size_t smem, bool& done) {
 }
 
 int launch_dr(const DrArgs& a, int nf, cudaStream_t st) {
-    dim3 grid((unsigned)((a.plane + DR_TB - 1) / DR_TB), nf);
+    dim3 grid((unsigned)((a.ncols + DR_TB - 1) / DR_TB), nf);
     k_dr<<<grid, DR_TB, 0, st>>>(a);
     return (int)cudaGetLastError();
 }

@@ -42,8 +42,8 @@ __global__ void __launch_bounds__(DR_TB) k_dr(DrArgs a) {
     __shared__ __align__(16) cd ring[16][DR_TB];
     const int tx = threadIdx.x;
     const size_t col0 = (size_t)blockIdx.x * DR_TB + tx;
-    const bool valid = col0 < a.plane;
-    const size_t col = valid ? col0 : a.plane - 1;
+    const bool valid = col0 < a.ncols;
+    const size_t col = valid ? col0 : a.ncols - 1;
     const int fi = blockIdx.y;
     const cd* src = (fi == 0 ? a.f[0] : fi == 1 ? a.f[1] : fi == 2 ? a.f[2] : a.f[3]) + col;
     cd* dst = (fi == 0 ? a.out[0] : fi == 1 ? a.out[1] : fi == 2 ? a.out[2] : a.out[3]) + col;
@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
     load_twiddles(tw, A.tw768);
     const int mtiles = a.MP / 4;
     const size_t plane = (size_t)a.M1 * a.NK;
-    const size_t qstride = (size_t)a.JC * N * a.MP;
+    const size_t qstride = (size_t)N * a.MP;
     const double taud = (double)tau;
     const int NKc = a.NK;
 
@@ -239,7 +239,7 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
                 for (int e = 0; e < 32; ++e) tile[tile4(p_idx(e, tau), warp)] = x[e];
             }
             __syncthreads();
-            cd* dst = a.zbuf + (size_t)(3 * fi + q) * qstride + (size_t)jl * N * a.MP + mt * 4;
+            cd* dst = a.zbuf + ((size_t)jl * 3 * a.nf + (3 * fi + q)) * qstride + mt * 4;
 #pragma unroll 4
             for (int it = 0; it < (N * 4) / Z2_THREADS; ++it) {
                 const int id = threadIdx.x + it * Z2_THREADS;
@@ -267,12 +267,12 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zfwd2(Nl2Args A) {
     load_twiddles(tw, A.tw768);
     const int a23 = tau < NA ? tau : NA - 1;
     const int mtiles = a.MP / 4;
-    const size_t qstride = (size_t)a.JC * N * a.MP;
+    const size_t qstride = (size_t)N * a.MP;
 
     auto fetch = [&](int it) {
         const int mt = it % mtiles, r = it / mtiles;
         const int jl = r % a.nj, fi = r / a.nj;
-        const cd* src = a.tbuf + (size_t)fi * qstride + (size_t)jl * N * a.MP + mt * 4;
+        const cd* src = a.tbuf + ((size_t)jl * a.nf + fi) * qstride + mt * 4;
 #pragma unroll 4
         for (int k = 0; k < (N * 4) / Z2_THREADS; ++k) {
             const int id = threadIdx.x + k * Z2_THREADS;
@@ -587,14 +587,14 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
     }
     const int M = a.M;
     const double taud = (double)tau, kth0 = A.ktheta0;
-    const size_t qstride = (size_t)a.JC * a.Nz * a.MP;
+    const size_t qstride = (size_t)a.Nz * a.MP;
     const int nlines = a.nj * a.Nz;
     const int lstride = gridDim.x * Cfg::WARPS;
     // this warp's staged line pair (X, Y) of the next inverse transform, filled by cp.async
     cd* stX = tw + XBUF * (1 + Cfg::WARPS) + 2 * T2_STAGE * warp;
     cd* stY = stX + T2_STAGE;
     auto stage = [&](int ln, int t) {
-        const size_t off = (size_t)ln * a.MP;
+        const size_t off = ((size_t)(ln / a.Nz) * 3 * a.nf * a.Nz + ln % a.Nz) * a.MP;
         const cd* X = a.zbuf + (size_t)t2_qx(t) * qstride + off;
         const cd* Y = a.zbuf + (size_t)t2_qy(t) * qstride + off;
         for (int i = tau; i <= M; i += 32) {
@@ -606,7 +606,7 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
     if (line < nlines) stage(line, 0);
     for (; line < nlines; line += lstride) {
         const int jl = line / a.Nz;
-        const size_t loff = (size_t)line * a.MP;               // (jl * Nz + z) * MP
+        const size_t loff = ((size_t)jl * a.nf * a.Nz + line % a.Nz) * a.MP;   // line (j, z) of q = 0 in tbuf
         const double ri = a.rinv[a.j0 + jl];
         const double rj = 1.0 / ri;
         cd x[32];

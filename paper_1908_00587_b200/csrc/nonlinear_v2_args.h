@@ -10,7 +10,8 @@ struct DrArgs {
     cd* out[MAXF];
     const double* D1;
     int N_r;
-    size_t plane;          // complex elements per radial level (M1 * NK)
+    size_t plane;          // stride between radial levels (complex elements)
+    size_t ncols;          // columns of one field per level (<= plane)
 };
 
 struct Nl2Args {

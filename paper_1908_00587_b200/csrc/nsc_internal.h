@@ -63,8 +63,8 @@ struct nsc_ctx {
     nsc::cd* DP = nullptr;                // D1 p of the state (fused linear path)
     nsc::cd* N0[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* N1[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
-    nsc::cd* zbuf = nullptr;              // [3 nf][JC][N_z][MP]  z-transformed f, dz f, dr f
-    nsc::cd* tbuf = nullptr;              // [nf][JC][N_z][MP]    theta-transformed products
+    nsc::cd* zbuf = nullptr;              // [JC][3 nf][N_z][MP]  z-transformed f, dz f, dr f
+    nsc::cd* tbuf = nullptr;              // [JC][nf][N_z][MP]    theta-transformed products
     nsc::cd* DR[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};       // D1 f (length-768 z pipeline)
     bool z768 = false;                    // z transforms by k_dr + k_zinv2 / k_zfwd2
     int t768 = 0;                         // theta transforms by k_theta2: 0 no, 1 shared-memory, 2 TMEM scratch
