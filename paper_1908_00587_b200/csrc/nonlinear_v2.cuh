@@ -512,19 +512,19 @@ __device__ __forceinline__ void prefetch_l2(const void* p) {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
 
-// run-time variant of load_pair768 (dx, dy select the d/dtheta multiplier i n): one copy of the code
-// serves all six inverse transforms of a point-line, which keeps the kernel inside the instruction cache
+// run-time variant of load_pair768: one copy of the code serves all six inverse transforms of a
+// point-line, which keeps the kernel inside the instruction cache.  dx / dy select the d/dtheta
+// multiplier i n of the X / Y half; the four transforms without a derivative take the short branch
+// (uniform per warp), the other two blend (1, 0) / (0, n) multipliers arithmetically (no selects).
 __device__ __forceinline__ void load_pair768_rt(cd* x, const cd* X, const cd* Y, bool dx, bool dy, int M, int tau,
                                                 double taud, double kth0) {
+    if (!(dx || dy)) {
 #define NSC_POS(T)                                                    \
     {                                                                 \
         const int m = tau + 32 * T;                                   \
         const bool ok = m <= M;                                       \
         cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
         cd gy = ok ? Y[m] : mk(0.0, 0.0);                             \
-        const double n = kth0 * (taud + (double)(32 * T));            \
-        if (dx) gx = n * mul_i(gx);                                   \
-        if (dy) gy = n * mul_i(gy);                                   \
         if (T == 0 && tau == 0) {                                     \
             gx.y = 0.0;                                               \
             gy.y = 0.0;                                               \
@@ -535,19 +535,53 @@ __device__ __forceinline__ void load_pair768_rt(cd* x, const cd* X, const cd* Y,
     {                                                                 \
         const int m = f768::N - 32 * T - tau;                         \
         const bool ok = m <= M;                                       \
-        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
-        cd gy = ok ? Y[m] : mk(0.0, 0.0);                             \
-        const double n = kth0 * ((double)(f768::N - 32 * T) - taud);  \
-        if (dx) gx = n * mul_i(gx);                                   \
-        if (dy) gy = n * mul_i(gy);                                   \
+        const cd gx = ok ? X[m] : mk(0.0, 0.0);                       \
+        const cd gy = ok ? Y[m] : mk(0.0, 0.0);                       \
         x[T] = mk(gx.x + gy.y, gy.x - gx.y);                          \
     }
-    NSC_POS(0) NSC_POS(1) NSC_POS(2) NSC_POS(3) NSC_POS(4) NSC_POS(5) NSC_POS(6) NSC_POS(7) NSC_POS(8)
-#pragma unroll
-    for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
-    NSC_NEG(16) NSC_NEG(17) NSC_NEG(18) NSC_NEG(19) NSC_NEG(20) NSC_NEG(21) NSC_NEG(22) NSC_NEG(23)
+        NSC_POS(0) NSC_POS(1) NSC_POS(2) NSC_POS(3) NSC_POS(4) NSC_POS(5) NSC_POS(6) NSC_POS(7) NSC_POS(8)
+        NSC_NEG(16) NSC_NEG(17) NSC_NEG(18) NSC_NEG(19) NSC_NEG(20) NSC_NEG(21) NSC_NEG(22) NSC_NEG(23)
 #undef NSC_POS
 #undef NSC_NEG
+    } else {
+        // g' = (a + i b n) g with (a, b) = (1, 0) plain or (0, 1) derivative
+        const double ax = dx ? 0.0 : 1.0, bx = dx ? kth0 : 0.0;
+        const double ay = dy ? 0.0 : 1.0, by = dy ? kth0 : 0.0;
+#define NSC_POS(T)                                                    \
+    {                                                                 \
+        const int m = tau + 32 * T;                                   \
+        const bool ok = m <= M;                                       \
+        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
+        cd gy = ok ? Y[m] : mk(0.0, 0.0);                             \
+        if (T == 0 && tau == 0) {                                     \
+            gx.y = 0.0;                                               \
+            gy.y = 0.0;                                               \
+        }                                                             \
+        const double mr = taud + (double)(32 * T);                    \
+        const double bxn = bx * mr, byn = by * mr;                    \
+        const cd hx = mk(fma(-bxn, gx.y, ax * gx.x), fma(bxn, gx.x, ax * gx.y)); \
+        const cd hy = mk(fma(-byn, gy.y, ay * gy.x), fma(byn, gy.x, ay * gy.y)); \
+        x[T] = mk(hx.x - hy.y, hx.y + hy.x);                          \
+    }
+#define NSC_NEG(T)                                                    \
+    {                                                                 \
+        const int m = f768::N - 32 * T - tau;                         \
+        const bool ok = m <= M;                                       \
+        const cd gx = ok ? X[m] : mk(0.0, 0.0);                       \
+        const cd gy = ok ? Y[m] : mk(0.0, 0.0);                       \
+        const double mr = (double)(f768::N - 32 * T) - taud;          \
+        const double bxn = bx * mr, byn = by * mr;                    \
+        const cd hx = mk(fma(-bxn, gx.y, ax * gx.x), fma(bxn, gx.x, ax * gx.y)); \
+        const cd hy = mk(fma(-byn, gy.y, ay * gy.x), fma(byn, gy.x, ay * gy.y)); \
+        x[T] = mk(hx.x + hy.y, hy.x - hx.y);                          \
+    }
+        NSC_POS(0) NSC_POS(1) NSC_POS(2) NSC_POS(3) NSC_POS(4) NSC_POS(5) NSC_POS(6) NSC_POS(7) NSC_POS(8)
+        NSC_NEG(16) NSC_NEG(17) NSC_NEG(18) NSC_NEG(19) NSC_NEG(20) NSC_NEG(21) NSC_NEG(22) NSC_NEG(23)
+#undef NSC_POS
+#undef NSC_NEG
+    }
+#pragma unroll
+    for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
 }
 
 // The six inverse transforms of a point-line as a table: work array index q = 3 field + kind
