@@ -342,8 +342,8 @@ struct TmemScratch {
             "r"(__double2hiint(v[7]))
             : "memory");
     }
-    __device__ __forceinline__ void ld8(uint32_t addr, double* v) const {
-        uint32_t r[16];
+    // asynchronous: the 16 raw registers are valid only after wait_ld()
+    __device__ __forceinline__ void ld8_raw(uint32_t addr, uint32_t* r) const {
         asm volatile(
             "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, "
             "%14, %15}, [%16];"
@@ -351,10 +351,16 @@ struct TmemScratch {
               "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
             : "r"(addr)
             : "memory");
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    }
+    __device__ __forceinline__ void ld8(uint32_t addr, double* v) const {
+        uint32_t r[16];
+        ld8_raw(addr, r);
+        wait_ld();
 #pragma unroll
         for (int i = 0; i < 8; ++i) v[i] = __hiloint2double((int)r[2 * i + 1], (int)r[2 * i]);
     }
+    // the registers of every ld8 issued so far are valid after this
+    __device__ __forceinline__ void wait_ld() const { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
     __device__ __forceinline__ void st(int slot, const double* v) const {
 #pragma unroll
         for (int c = 0; c < 4; ++c) st8(base + slot * 64 + c * 16, v + 8 * c);
@@ -417,6 +423,27 @@ __device__ __forceinline__ void sc_ld8(const SmemScratch& s, int slot, int c, do
     for (int i = 0; i < 8; ++i) v[i] = s.base[(slot * 32 + c * 8 + i) * f768::NA];
 }
 __device__ __forceinline__ void sc_fence(const SmemScratch&) {}
+// split form: sc_ld8_raw (issue) ... sc_wait_ld ... sc_unpack8 (use), so that several loads share one wait
+struct Raw8 {
+    uint32_t r[16];
+};
+__device__ __forceinline__ void sc_ld8_raw(const TmemScratch& s, int slot, int c, Raw8& q) {
+    s.ld8_raw(s.base + slot * 64 + c * 16, q.r);
+}
+__device__ __forceinline__ void sc_ld8_raw(const SmemScratch& s, int slot, int c, Raw8& q) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const double v = s.base[(slot * 32 + c * 8 + i) * f768::NA];
+        q.r[2 * i] = (uint32_t)__double2loint(v);
+        q.r[2 * i + 1] = (uint32_t)__double2hiint(v);
+    }
+}
+__device__ __forceinline__ void sc_wait_ld(const TmemScratch& s) { s.wait_ld(); }
+__device__ __forceinline__ void sc_wait_ld(const SmemScratch&) {}
+__device__ __forceinline__ void sc_unpack8(const Raw8& q, double* v) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __hiloint2double((int)q.r[2 * i + 1], (int)q.r[2 * i]);
+}
 
 // ------------------------------------------------------------------------------------------ k_theta2
 // Z[i] = G_X(i) + i G_Y(i) in the S layout, G(m) = mult * line[m] (0 <= m <= M), G(-m) = conj G(m),
@@ -674,7 +701,10 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t2[8];
-                    sc_ld8(sc, 0, c, t0);
+                    Raw8 q0;
+                    sc_ld8_raw(sc, 0, c, q0);
+                    sc_wait_ld(sc);
+                    sc_unpack8(q0, t0);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         t2[i] = x[8 * c + i].x;
@@ -686,8 +716,13 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t1[8], t2[8];
-                    sc_ld8(sc, 1, c, t1);
-                    sc_ld8(sc, 2, c, t2);
+                    Raw8 q0;
+                    Raw8 q1;
+                    sc_ld8_raw(sc, 1, c, q0);
+                    sc_ld8_raw(sc, 2, c, q1);
+                    sc_wait_ld(sc);
+                    sc_unpack8(q0, t1);
+                    sc_unpack8(q1, t2);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         double s = fma(t1[i], x[8 * c + i].x, acc[8 * c + i]);
@@ -701,8 +736,13 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t1[8];
-                    sc_ld8(sc, 0, c, t0);
-                    sc_ld8(sc, 1, c, t1);
+                    Raw8 q0;
+                    Raw8 q1;
+                    sc_ld8_raw(sc, 0, c, q0);
+                    sc_ld8_raw(sc, 1, c, q1);
+                    sc_wait_ld(sc);
+                    sc_unpack8(q0, t0);
+                    sc_unpack8(q1, t1);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) acc[8 * c + i] = fma(t1[i], x[8 * c + i].y, t0[i] * x[8 * c + i].x);
                 }
@@ -710,10 +750,19 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t1[8], t2[8], t3[8];
-                    sc_ld8(sc, 0, c, t0);
-                    sc_ld8(sc, 1, c, t1);
-                    sc_ld8(sc, 2, c, t2);
-                    sc_ld8(sc, 3, c, t3);
+                    Raw8 q0;
+                    Raw8 q1;
+                    Raw8 q2;
+                    Raw8 q3;
+                    sc_ld8_raw(sc, 0, c, q0);
+                    sc_ld8_raw(sc, 1, c, q1);
+                    sc_ld8_raw(sc, 2, c, q2);
+                    sc_ld8_raw(sc, 3, c, q3);
+                    sc_wait_ld(sc);
+                    sc_unpack8(q0, t0);
+                    sc_unpack8(q1, t1);
+                    sc_unpack8(q2, t2);
+                    sc_unpack8(q3, t3);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         double s = fma(t2[i], x[8 * c + i].x, acc[8 * c + i]);
@@ -727,9 +776,16 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t1[8], t2[8];
-                    sc_ld8(sc, 1, c, t1);
-                    sc_ld8(sc, 2, c, t2);
-                    sc_ld8(sc, 3, c, t0);
+                    Raw8 q0;
+                    Raw8 q1;
+                    Raw8 q2;
+                    sc_ld8_raw(sc, 1, c, q0);
+                    sc_ld8_raw(sc, 2, c, q1);
+                    sc_ld8_raw(sc, 3, c, q2);
+                    sc_wait_ld(sc);
+                    sc_unpack8(q0, t1);
+                    sc_unpack8(q1, t2);
+                    sc_unpack8(q2, t0);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         double s = fma(t1[i], x[8 * c + i].x, t0[i]);
