@@ -86,10 +86,10 @@ LINEAR_KERNELS = ("k_rhs_fwd", "k_bwd_div", "k_poisson_fwd", "k_poisson_bwd_corr
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r01_final_ncu_full.md), cfg 4, full 55-level radial chunk; None where no capture exists
+# (profiles/r01_final_ncu_full.md), cfg 4, one launch = all 256 radial levels; None where no capture exists
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    ("k_theta", 4): 1.610609e9 + 0.519734e9,
-    ("k_zinv", 4): 0.696259e9 + 1.554979e9,
+    ("k_theta", 4): 7.498633e9 + 2.536703e9,
+    ("k_zinv", 4): 1.620360e9 + 4.930793e9,
 }
 
 
