@@ -862,13 +862,11 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
         fa.DP = c->DP;
         fa.offL4 = c->shH.h_offL[FWI];
         fa.offU4 = c->shH.h_offU[FWI];
-        static bool attr_done = false;
-        if (!attr_done) {
+        {   // per device, so set on every launch (a few microseconds)
             cudaFuncSetAttribute(k_rhs_fwd<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_F * sizeof(FwdSlot<3>)));
             cudaFuncSetAttribute(k_rhs_fwd<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_F * sizeof(FwdSlot<4>)));
             cudaFuncSetAttribute(k_bwd_div<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_B * sizeof(BwdSlot<3>)));
             cudaFuncSetAttribute(k_bwd_div<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_B * sizeof(BwdSlot<4>)));
-            attr_done = true;
         }
         prof_begin(c, NSC_K_RHS);
         if (c->nf == 3)
@@ -914,11 +912,9 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
         pa.nf = c->nf;
         pa.copyT = (c->nf == 4 && dst[3] != c->W[3]) ? 1 : 0;
         pa.dt = dt;
-        static bool pattr_done = false;
-        if (!pattr_done) {
+        {
             cudaFuncSetAttribute(k_poisson_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_PF * sizeof(PFwdSlot)));
             cudaFuncSetAttribute(k_poisson_bwd_correct, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_PB * sizeof(PBwdSlot)));
-            pattr_done = true;
         }
         prof_begin(c, NSC_K_POISSON);
         k_poisson_fwd<<<(plane + PBP - 1) / PBP, PBP, PIPE_PF * sizeof(PFwdSlot), c->stream>>>(pa);

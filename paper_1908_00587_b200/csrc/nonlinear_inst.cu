@@ -13,15 +13,10 @@ namespace nsc {
 #define NSC_CAT(a, b) NSC_CAT2(a, b)
 constexpr int LEN = NSC_FFT_N;
 
-// raises the dynamic shared-memory limit of kernel k once (ID = one flag per kernel)
+// raises the dynamic shared-memory limit of kernel k (a per-device attribute: set on every launch)
 template <int ID, class Kern> static int prep(Kern k, size_t smem) {
-    static bool done = false;
-    if (!done) {
-        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
-        done = true;
-    }
-    return 0;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return e == cudaSuccess ? 0 : (int)e;
 }
 
 int NSC_CAT(launch_zinv_, NSC_FFT_N)(const NlArgs& a, cudaStream_t st) {

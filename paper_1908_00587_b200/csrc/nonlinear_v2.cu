@@ -14,13 +14,10 @@ static int sm_count() {
     return n;
 }
 
-template <class Kern> static int set_smem(Kern k, size_t smem, bool& done) {
-    if (!done) {
-        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
-        done = true;
-    }
-    return 0;
+// the attribute is per device: set on every launch (a few microseconds) rather than cached per process
+template <class Kern> static int set_smem(Kern k, size_t smem) {
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    return e == cudaSuccess ? 0 : (int)e;
 }
 
 int launch_dr(const DrArgs& a, int nf, cudaStream_t st) {
@@ -30,8 +27,7 @@ int launch_dr(const DrArgs& a, int nf, cudaStream_t st) {
 }
 
 int launch_zinv2(const Nl2Args& a, cudaStream_t st) {
-    static bool done = false;
-    if (int e = set_smem(k_zinv2, Z2_SMEM_INV, done)) return e;
+    if (int e = set_smem(k_zinv2, Z2_SMEM_INV)) return e;
     int grid = 2 * sm_count();
     if (grid > a.nitems) grid = a.nitems;
     k_zinv2<<<grid, Z2_THREADS, Z2_SMEM_INV, st>>>(a);
@@ -39,8 +35,7 @@ int launch_zinv2(const Nl2Args& a, cudaStream_t st) {
 }
 
 int launch_zfwd2(const Nl2Args& a, cudaStream_t st) {
-    static bool done = false;
-    if (int e = set_smem(k_zfwd2, Z2_SMEM_FWD, done)) return e;
+    if (int e = set_smem(k_zfwd2, Z2_SMEM_FWD)) return e;
     int grid = 2 * sm_count();
     if (grid > a.nitems) grid = a.nitems;
     k_zfwd2<<<grid, Z2_THREADS, Z2_SMEM_FWD, st>>>(a);
@@ -51,15 +46,13 @@ int launch_theta2(const Nl2Args& a, bool tmem, cudaStream_t st) {
     const int nlines = a.b.nj * a.b.Nz;
     if (tmem) {
         using C = T2Cfg<true>;
-        static bool done = false;
-        if (int e = set_smem(k_theta2<true>, C::SMEM, done)) return e;
+            if (int e = set_smem(k_theta2<true>, C::SMEM)) return e;
         int grid = sm_count();
         if (grid > (nlines + C::WARPS - 1) / C::WARPS) grid = (nlines + C::WARPS - 1) / C::WARPS;
         k_theta2<true><<<grid, C::WARPS * 32, C::SMEM, st>>>(a);
     } else {
         using C = T2Cfg<false>;
-        static bool done = false;
-        if (int e = set_smem(k_theta2<false>, C::SMEM, done)) return e;
+            if (int e = set_smem(k_theta2<false>, C::SMEM)) return e;
         int grid = sm_count();
         if (grid > (nlines + C::WARPS - 1) / C::WARPS) grid = (nlines + C::WARPS - 1) / C::WARPS;
         k_theta2<false><<<grid, C::WARPS * 32, C::SMEM, st>>>(a);
