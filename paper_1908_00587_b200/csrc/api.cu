@@ -157,6 +157,13 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
         if (!rc) rc = dev_alloc(c, &c->zbuf, (size_t)3 * c->nf * c->JC * c->Nz * c->MP, true);
         if (!rc) rc = dev_alloc(c, &c->tbuf, (size_t)c->nf * c->JC * c->Nz * c->MP, true);
     }
+    if (const char* ev = getenv("NSC_LIN_SLICES")) c->n_slices = atoi(ev);
+    if (c->n_slices < 1) c->n_slices = 1;
+    if (c->n_slices > NSC_MAX_SLICES) c->n_slices = NSC_MAX_SLICES;
+    for (int i = 0; i < c->n_slices && !rc && c->n_slices > 1; ++i)
+        if (cudaStreamCreateWithFlags(&c->slice_stream[i], cudaStreamNonBlocking) != cudaSuccess) rc = fail(c, NSC_ECUDA, "cudaStreamCreate");
+    for (int i = 0; i <= c->n_slices && !rc; ++i)
+        if (cudaEventCreateWithFlags(&c->slice_ev[i], cudaEventDisableTiming) != cudaSuccess) rc = fail(c, NSC_ECUDA, "cudaEventCreate");
     if (!rc) {
         e = cudaDeviceSynchronize();
         if (e != cudaSuccess) rc = cuda_fail(c, e, "nsc_create: cudaDeviceSynchronize");
@@ -198,6 +205,10 @@ int nsc_destroy(nsc_ctx* c) {
         cudaEventDestroy(r.b);
     }
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    for (cudaStream_t s : c->slice_stream)
+        if (s) cudaStreamDestroy(s);
+    for (cudaEvent_t e : c->slice_ev)
+        if (e) cudaEventDestroy(e);
     cudaGetLastError();
     delete c;
     return NSC_OK;

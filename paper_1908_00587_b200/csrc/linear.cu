@@ -116,6 +116,7 @@ struct FusedArgs {
     const int* s0;
     int N_r, M1, NK, K, P, nf;
     int offL4, offU4;      // offL[4], offU[4]: the interior rows 4 .. N_r - 5 have regular offsets
+    int e_begin, e_end;    // slice of modes [e_begin, e_end) this launch serves
     double dt, c, w0, w1, Re_i, Re_o;
 };
 
@@ -191,9 +192,9 @@ __global__ void __launch_bounds__(PBK * NF, NSC_K1_MINB) k_rhs_fwd(FusedArgs a) 
     FwdSlot<NF>* slots = reinterpret_cast<FwdSlot<NF>*>(smem_raw);
     const int tx = threadIdx.x, fld = threadIdx.y;
     const int plane_i = a.M1 * a.NK;
-    const int e0 = blockIdx.x * PBK + tx;
-    const bool valid = e0 < plane_i;
-    const int e = valid ? e0 : plane_i - 1;
+    const int e0 = a.e_begin + blockIdx.x * PBK + tx;
+    const bool valid = e0 < a.e_end;
+    const int e = valid ? e0 : a.e_end - 1;
     const int m = e / a.NK, kk = e % a.NK;
     const int ka = kk >= a.K ? kk - a.K : a.K - kk;
     const size_t P = a.P;
@@ -337,9 +338,9 @@ __global__ void __launch_bounds__(PBK * (NF + 1), NF == 3 ? NSC_K2_MINB : 3) k_b
     __shared__ cd ring_g[FW][PBK];                      // divergence-role thread tx), stencil-free part of g
     const int tx = threadIdx.x, role = threadIdx.y;
     const int plane_i = a.M1 * a.NK;
-    const int e0 = blockIdx.x * PBK + tx;
-    const bool valid = e0 < plane_i;
-    const int e = valid ? e0 : plane_i - 1;
+    const int e0 = a.e_begin + blockIdx.x * PBK + tx;
+    const bool valid = e0 < a.e_end;
+    const int e = valid ? e0 : a.e_end - 1;
     const int m = e / a.NK, kk = e % a.NK;
     const int ka = kk >= a.K ? kk - a.K : a.K - kk;
     const size_t P = a.P;
@@ -495,6 +496,7 @@ struct PoisArgs {
     const int* s0;
     int N_r, M1, NK, K, P, nf;
     int copyT;             // dst[3] != W[3]
+    int e_begin, e_end;    // slice of modes [e_begin, e_end) this launch serves
     double dt;
 };
 
@@ -519,9 +521,9 @@ __global__ void __launch_bounds__(PBP) k_poisson_fwd(PoisArgs a) {
     PFwdSlot* slots = reinterpret_cast<PFwdSlot*>(smem_raw);
     const int tx = threadIdx.x;
     const int plane_i = a.M1 * a.NK;
-    const int e0 = blockIdx.x * PBP + tx;
-    const bool valid = e0 < plane_i;
-    const int e = valid ? e0 : plane_i - 1;
+    const int e0 = a.e_begin + blockIdx.x * PBP + tx;
+    const bool valid = e0 < a.e_end;
+    const int e = valid ? e0 : a.e_end - 1;
     const int m = e / a.NK, kk = e % a.NK;
     const int ka = kk >= a.K ? kk - a.K : a.K - kk;
     const size_t P = a.P;
@@ -594,9 +596,9 @@ __global__ void __launch_bounds__(PBB) k_poisson_bwd_correct(PoisArgs a) {
     PBwdSlot* slots = reinterpret_cast<PBwdSlot*>(smem_raw);
     const int tx = threadIdx.x;
     const int plane_i = a.M1 * a.NK;
-    const int e0 = blockIdx.x * PBB + tx;
-    const bool valid = e0 < plane_i;
-    const int e = valid ? e0 : plane_i - 1;
+    const int e0 = a.e_begin + blockIdx.x * PBB + tx;
+    const bool valid = e0 < a.e_end;
+    const int e = valid ? e0 : a.e_end - 1;
     const int m = e / a.NK, kk = e % a.NK;
     const int ka = kk >= a.K ? kk - a.K : a.K - kk;
     const size_t P = a.P;
@@ -858,7 +860,6 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
         fa.w1 = w1;
         fa.Re_i = c->p.Re_i;
         fa.Re_o = c->p.Re_o;
-        const int nb = (plane + PBK - 1) / PBK;
         fa.DP = c->DP;
         fa.offL4 = c->shH.h_offL[FWI];
         fa.offU4 = c->shH.h_offU[FWI];
@@ -868,20 +869,6 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
             cudaFuncSetAttribute(k_bwd_div<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_B * sizeof(BwdSlot<3>)));
             cudaFuncSetAttribute(k_bwd_div<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_B * sizeof(BwdSlot<4>)));
         }
-        prof_begin(c, NSC_K_RHS);
-        if (c->nf == 3)
-            k_rhs_fwd<3><<<nb, dim3(PBK, 3), PIPE_F * sizeof(FwdSlot<3>), c->stream>>>(fa);
-        else
-            k_rhs_fwd<4><<<nb, dim3(PBK, 4), PIPE_F * sizeof(FwdSlot<4>), c->stream>>>(fa);
-        prof_end(c);
-        NSC_CUDA(c, cudaGetLastError());
-        prof_begin(c, NSC_K_HELMHOLTZ);
-        if (c->nf == 3)
-            k_bwd_div<3><<<nb, dim3(PBK, 4), PIPE_B * sizeof(BwdSlot<3>), c->stream>>>(fa);
-        else
-            k_bwd_div<4><<<nb, dim3(PBK, 5), PIPE_B * sizeof(BwdSlot<4>), c->stream>>>(fa);
-        prof_end(c);
-        NSC_CUDA(c, cudaGetLastError());
         PoisArgs pa{};
         pa.G = c->G;
         pa.L = c->facP.L;
@@ -916,14 +903,51 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
             cudaFuncSetAttribute(k_poisson_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_PF * sizeof(PFwdSlot)));
             cudaFuncSetAttribute(k_poisson_bwd_correct, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(PIPE_PB * sizeof(PBwdSlot)));
         }
-        prof_begin(c, NSC_K_POISSON);
-        k_poisson_fwd<<<(plane + PBP - 1) / PBP, PBP, PIPE_PF * sizeof(PFwdSlot), c->stream>>>(pa);
-        prof_end(c);
-        NSC_CUDA(c, cudaGetLastError());
-        prof_begin(c, NSC_K_CORRECT);
-        k_poisson_bwd_correct<<<(plane + PBB - 1) / PBB, PBB, PIPE_PB * sizeof(PBwdSlot), c->stream>>>(pa);
-        prof_end(c);
-        NSC_CUDA(c, cudaGetLastError());
+        // The four sweeps of a block of modes depend only on each other, so the mode range is cut into slices
+        // whose kernel chains run on separate streams: while one slice's sweep drains (a march has no work
+        // left for the SMs its finished columns occupied), the next sweep of the other slice fills the machine.
+        // With per-kernel profiling on, one slice on the caller's stream (the event brackets need one stream).
+        const int nsl = (c->profiling || !c->slice_stream[0]) ? 1 : c->n_slices;
+        const int per = ((plane + nsl - 1) / nsl + 127) / 128 * 128;       // multiple of every block width
+        if (nsl > 1) {
+            NSC_CUDA(c, cudaEventRecord(c->slice_ev[0], c->stream));
+        }
+        for (int sl = 0; sl < nsl; ++sl) {
+            const int eb = sl * per, ee = (eb + per < plane) ? eb + per : plane;
+            if (eb >= ee) continue;
+            cudaStream_t st = (nsl > 1) ? c->slice_stream[sl] : c->stream;
+            if (nsl > 1) NSC_CUDA(c, cudaStreamWaitEvent(st, c->slice_ev[0], 0));
+            fa.e_begin = pa.e_begin = eb;
+            fa.e_end = pa.e_end = ee;
+            const int ne = ee - eb;
+            const int nb = (ne + PBK - 1) / PBK;
+            prof_begin(c, NSC_K_RHS);
+            if (c->nf == 3)
+                k_rhs_fwd<3><<<nb, dim3(PBK, 3), PIPE_F * sizeof(FwdSlot<3>), st>>>(fa);
+            else
+                k_rhs_fwd<4><<<nb, dim3(PBK, 4), PIPE_F * sizeof(FwdSlot<4>), st>>>(fa);
+            prof_end(c);
+            NSC_CUDA(c, cudaGetLastError());
+            prof_begin(c, NSC_K_HELMHOLTZ);
+            if (c->nf == 3)
+                k_bwd_div<3><<<nb, dim3(PBK, 4), PIPE_B * sizeof(BwdSlot<3>), st>>>(fa);
+            else
+                k_bwd_div<4><<<nb, dim3(PBK, 5), PIPE_B * sizeof(BwdSlot<4>), st>>>(fa);
+            prof_end(c);
+            NSC_CUDA(c, cudaGetLastError());
+            prof_begin(c, NSC_K_POISSON);
+            k_poisson_fwd<<<(ne + PBP - 1) / PBP, PBP, PIPE_PF * sizeof(PFwdSlot), st>>>(pa);
+            prof_end(c);
+            NSC_CUDA(c, cudaGetLastError());
+            prof_begin(c, NSC_K_CORRECT);
+            k_poisson_bwd_correct<<<(ne + PBB - 1) / PBB, PBB, PIPE_PB * sizeof(PBwdSlot), st>>>(pa);
+            prof_end(c);
+            NSC_CUDA(c, cudaGetLastError());
+            if (nsl > 1) {
+                NSC_CUDA(c, cudaEventRecord(c->slice_ev[1 + sl], st));
+                NSC_CUDA(c, cudaStreamWaitEvent(c->stream, c->slice_ev[1 + sl], 0));
+            }
+        }
     }
     return NSC_OK;
 }

@@ -48,6 +48,8 @@ struct Tables {               // all device pointers
 
 }  // namespace nsc
 
+constexpr int NSC_MAX_SLICES = 8;
+
 struct nsc_ctx {
     nsc_params p{};
     int N_r = 0, M = 0, K = 0, M1 = 0, NK = 0, MP = 0, Nt = 0, Nz = 0, nf = 3, JC = 0;
@@ -74,6 +76,9 @@ struct nsc_ctx {
     bool facT_shared = false;             // T shares the u_z factors (Pr == 1)
     double fac_dt = 0.0;                  // dt the Helmholtz factors were built for (0: none)
     bool facP_ready = false;
+    int n_slices = 2;                                 // mode slices of the linear stage (NSC_LIN_SLICES overrides)
+    cudaStream_t slice_stream[NSC_MAX_SLICES] = {};   // their streams
+    cudaEvent_t slice_ev[NSC_MAX_SLICES + 1] = {};    // [0] fork, [1 + s] join of slice s
     bool have_state = false;
     std::string err;
     long long launches = 0;
