@@ -62,7 +62,8 @@ typedef struct nsc_params {
                          in {12,24,...,1536} that are >= the 3/2 rule                              */
     double c;         /* implicitness of the linear terms; 0 => 0.5 (R10)                         */
     int device;       /* CUDA device ordinal; -1 => current device                                */
-    int radial_chunk; /* radial nodes per pass of the transform pipeline; 0 => automatic          */
+    int radial_chunk; /* radial nodes per pass of the transform pipeline; 0 => automatic (all N_r
+                       * at once when the work arrays fit an eighth of the device memory)         */
 } nsc_params;
 
 /* BJ: nsc_create(N_r, M_theta, K_z, eta, alpha, k_theta0, Re_i, Re_o, Ra, Pr, radial-grid type).
@@ -82,8 +83,10 @@ int nsc_set_stream(nsc_ctx* ctx, void* cuda_stream);
 /* Radial nodes r_j, j = 0..N_r-1, written to h_r (host, N_r doubles). */
 int nsc_get_grid(const nsc_ctx* ctx, double* h_r);
 
-/* Copies a state into the context (device-to-device on the stream).  d_T required iff Ra != 0;
- * d_p may be NULL (p = 0).  Each pointer: one spectral field as described above. */
+/* Copies a state into the context (device-to-device on the stream) and derives D1 p of it (one
+ * kernel launch; the linear stage keeps the radial pressure gradient as an array, DESIGN.md
+ * section 6).  d_T required iff Ra != 0; d_p may be NULL (p = 0).  Each pointer: one spectral
+ * field as described above. */
 int nsc_set_state(nsc_ctx* ctx, const void* d_ur, const void* d_uth, const void* d_uz,
                   const void* d_T, const void* d_p);
 /* Copies the current state out; NULL pointers are skipped. */
