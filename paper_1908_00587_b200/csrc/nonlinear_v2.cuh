@@ -240,11 +240,18 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
             }
             __syncthreads();
             cd* dst = a.zbuf + ((size_t)jl * 3 * a.nf + (3 * fi + q)) * qstride + mt * 4;
-#pragma unroll 4
-            for (int it = 0; it < (N * 4) / Z2_THREADS; ++it) {
-                const int id = threadIdx.x + it * Z2_THREADS;
-                const int z = id >> 2, c = id & 3;
-                dst[(size_t)z * a.MP + (c ^ ((z >> 1) & 3))] = tile[id];
+            // all shared-memory reads first, then all stores (the transform's registers are free here): no
+            // store has to release its source registers before the next read can issue
+            {
+                constexpr int NIT = (N * 4) / Z2_THREADS;       // 24
+                cd v[NIT];
+#pragma unroll
+                for (int it = 0; it < NIT; ++it) v[it] = tile[threadIdx.x + it * Z2_THREADS];
+                // id = threadIdx.x + 128 it: z = id >> 2 = (threadIdx.x >> 2) + 32 it, c = id & 3 = threadIdx.x & 3
+                const int z0 = threadIdx.x >> 2, c0 = threadIdx.x & 3;
+                cd* d0 = dst + (size_t)z0 * a.MP + (c0 ^ ((z0 >> 1) & 3));  // (z >> 1) & 3 is the same for z0 + 32 it
+#pragma unroll
+                for (int it = 0; it < NIT; ++it) d0[(size_t)(32 * it) * a.MP] = v[it];
             }
             __syncthreads();                            // tile free again
         }
