@@ -384,6 +384,30 @@ class Oracle:
         N1 = self.nonlinear(*s1[:nf])
         return self.substep(state, [c * a + (1 - c) * b for a, b in zip(N1, N0)], dt)
 
+    # ---------------------------------------------------------------- NEXT-1: iterated corrector
+    def step_iterated(self, state, dt, tol, max_corr):
+        """Predictor-corrector step with the corrector ITERATED to convergence (the reason
+        the paper gives for a predictor-corrector scheme is that it allows "a variable time step size with
+        dynamic control"; its ref. [6] is not available, so the stopping rule is DESIGN.md reading R16):
+            u^(1) = substep(N0),   u^(k+1) = substep(c N(u^(k)) + (1-c) N0),  k = 1, 2, ...
+        every sub-step starting from (u^n, T^n, p^n); stop after pass k when
+            err_k = ||u^(k+1) - u^(k)||_2 / ||u^(k+1)||_2 <= tol   (all nf fields concatenated)
+        or k = max_corr.  Returns (state, k, err_k).  max_corr = 1 is ``step`` (err is still reported)."""
+        c = self.p.c
+        nf = 4 if self.p.heated else 3
+        N0 = self.nonlinear(*state[:nf])
+        cur = self.substep(state, N0, dt)
+        k, err = 0, float("inf")
+        while k < max_corr:
+            Nk = self.nonlinear(*cur[:nf])
+            new = self.substep(state, [c * a + (1 - c) * b for a, b in zip(Nk, N0)], dt)
+            k += 1
+            err = rel_l2(cur[:nf], new[:nf])
+            cur = new
+            if err <= tol:
+                break
+        return cur, k, err
+
     # ---------------------------------------------------------------- basic states
     def zeros(self):
         p = self.p

@@ -232,3 +232,62 @@ def test_cfg1_twenty_steps_stable_and_divergence_free():
         st = o.step(st, cfg["dt"])
     assert scaled_div(o, *st[:3]) < 1e-11
     assert 0.5 < np.linalg.norm(st[0]) / e0 < 2.0
+
+
+# ---------------------------------------------------------------- NEXT-1: iterated corrector (R16)
+def _small_state(seed_cfg=0, N_r=16, M=4, K=4, amp=None):
+    from paper_1908_00587_b200 import synth
+    from helpers import oracle_of
+    cfg = synth.scaled_config(seed_cfg, N_r=N_r, M=M, K=K)
+    if amp is not None:
+        cfg["amp"] = amp
+    o = oracle_of(cfg, dft="fft")
+    return cfg, o, synth.make_state(cfg, o.r)
+
+
+def test_iterated_corrector_one_pass_is_the_plain_step():
+    cfg, o, st = _small_state()
+    a = o.step(st, cfg["dt"])
+    b, k, err = o.step_iterated(st, cfg["dt"], tol=0.0, max_corr=1)
+    assert k == 1 and np.isfinite(err)
+    for x, y in zip(a, b):
+        if x is not None:
+            np.testing.assert_array_equal(x, y)
+
+
+def test_iterated_corrector_converges_to_its_fixed_point():
+    """The limit of the iteration solves u = substep(c N(u) + (1-c) N0): the residual of that equation
+    at the returned state is of the order of the last increment, the increments contract geometrically,
+    and a tighter tolerance costs more passes."""
+    import numpy as np
+    from oracle.nsc_oracle import rel_l2
+    cfg, o, st = _small_state(amp=5e-2)
+    dt = 4 * cfg["dt"]
+    errs = []
+    for mc in (1, 2, 3, 4):
+        _, k, e = o.step_iterated(st, dt, tol=0.0, max_corr=mc)
+        assert k == mc
+        errs.append(e)
+    assert errs[1] < 0.5 * errs[0] and errs[2] < 0.5 * errs[1] and errs[3] < 0.5 * errs[2]
+    out, k, e = o.step_iterated(st, dt, tol=1e-10, max_corr=50)
+    assert e <= 1e-10 and k < 50
+    _, k_loose, _ = o.step_iterated(st, dt, tol=1e-6, max_corr=50)
+    assert k_loose < k
+    # fixed-point residual
+    c = o.p.c
+    N0 = o.nonlinear(*st[:3])
+    Nk = o.nonlinear(*out[:3])
+    again = o.substep(st, [c * a + (1 - c) * b for a, b in zip(Nk, N0)], dt)
+    assert rel_l2(again[:3], out[:3]) <= 1e-9
+
+
+def test_iterated_corrector_leaves_couette_flow_alone():
+    from paper_1908_00587_b200 import synth
+    from helpers import oracle_of
+    from oracle.nsc_oracle import rel_l2
+    cfg = synth.scaled_config(0, N_r=24, M=4, K=4)
+    o = oracle_of(cfg, dft="fft")
+    base = o.base_state_discrete()
+    out, k, err = o.step_iterated(base, 1e-2, tol=1e-12, max_corr=5)
+    assert k == 1 and err <= 1e-12
+    assert rel_l2(out[:3], base[:3]) <= 1e-13
