@@ -115,6 +115,17 @@ int nsc_substep(nsc_ctx* ctx, const void* d_Er, const void* d_Eth, const void* d
  *   per-mode banded matrices (kept until dt changes). */
 int nsc_step(nsc_ctx* ctx, double dt);
 
+/* The same step with the corrector iterated to convergence (PAPER.md:46
+ * "dynamic control" of the step size; stopping rule = DESIGN.md reading R16):
+ *   u^(1) = substep(N0);  u^(k+1) = substep(c N(u^(k)) + (1-c) N0), k = 1, 2, ..., every pass from
+ *   (u^n, T^n, p^n); stop after pass k when ||u^(k+1) - u^(k)||_2 / ||u^(k+1)||_2 <= tol (all
+ *   fields u_r, u_theta, u_z, (T) concatenated) or k = max_corr >= 1.
+ * The newest iterate and the pressure of its pass become the state.  *n_corr (may be NULL) receives
+ * k, *err (may be NULL) the last norm: a caller steers dt with them.  max_corr = 1 is nsc_step.
+ * Synchronises the stream once per pass (the norm is read back); the first call allocates
+ * (2 n_f + 2) more field-sized buffers. */
+int nsc_step_iterated(nsc_ctx* ctx, double dt, double tol, int max_corr, int* n_corr, double* err);
+
 /* Text of the last error of this context ("" if none); valid until the next call on ctx.
  * With ctx == NULL: the text of the last failed nsc_create on this thread. */
 const char* nsc_last_error(const nsc_ctx* ctx);
@@ -136,7 +147,7 @@ enum {
     NSC_K_ZFWD = 2,      /* N6: forward z-FFT, truncation, scaling, buoyancy                         */
     NSC_K_RHS = 3,       /* L1 + L2 (k_rhs_fwd): right-hand sides + forward substitution, marching up   */
     NSC_K_HELMHOLTZ = 4, /* L2 + L3 (k_bwd_div): back substitution, recombination, divergence, down     */
-    NSC_K_RECOMBINE = 5, /* (unused: fused into k_bwd_div)                                               */
+    NSC_K_RECOMBINE = 5, /* k_diff_norm: convergence norm of the iterated corrector (nsc_step_iterated)  */
     NSC_K_DIV = 6,       /* (unused: fused into k_bwd_div)                                               */
     NSC_K_POISSON = 7,   /* L4 (k_poisson_fwd): forward substitution of the pressure system, up          */
     NSC_K_CORRECT = 8,   /* L4 + L5 (k_poisson_bwd_correct): back substitution + correction, down        */

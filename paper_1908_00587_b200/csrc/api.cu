@@ -1,10 +1,12 @@
 // api.cu -- the C ABI of include/nsc.h: argument checks, allocation, and the composition of
 // one predictor-corrector step (O7) from the kernels of nonlinear.cu
 // and linear.cu.  No arithmetic of the method happens on the host after nsc_create.
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <utility>
 #include "nsc_internal.h"
 
 namespace nsc {
@@ -66,7 +68,7 @@ void prof_end(nsc_ctx* c) {
 }
 
 static const char* kKernelNames[NSC_NKERN] = {"k_zinv", "k_theta", "k_zfwd", "k_rhs_fwd", "k_bwd_div",
-                                              "(unused)", "(unused)", "k_poisson_fwd", "k_poisson_bwd_correct",
+                                              "k_diff_norm", "(unused)", "k_poisson_fwd", "k_poisson_bwd_correct",
                                               "k_factor", "k_dr"};
 
 static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
@@ -316,6 +318,50 @@ int nsc_step(nsc_ctx* c, double dt) {
     // N1 = N(u^1);  u^{n+1} = substep(c N1 + (1 - c) N0) from (u^n, p^n), in place
     if ((rc = launch_nonlinear(c, c->W, c->N1))) return rc;
     return launch_substep(c, c->N1, c->p.c, c->N0, 1.0 - c->p.c, dt, c->state, c->state[4]);
+}
+
+int nsc_step_iterated(nsc_ctx* c, double dt, double tol, int max_corr, int* n_corr, double* err) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_step_iterated before nsc_set_state");
+    if (!(dt > 0.0)) return fail(c, NSC_EINVAL, "nsc_step_iterated: dt must be > 0");
+    if (!(tol >= 0.0) || max_corr < 1) return fail(c, NSC_EINVAL, "nsc_step_iterated: tol must be >= 0 and max_corr >= 1");
+    int rc;
+    if (!c->it_acc) {                                    // first use: ping-pong iterates + pressure of a pass
+        for (int i = 0; i < c->nf; ++i) {
+            if ((rc = dev_alloc(c, &c->itA[i], c->F, false))) return rc;
+            if ((rc = dev_alloc(c, &c->itB[i], c->F, false))) return rc;
+        }
+        if ((rc = dev_alloc(c, &c->itP, c->F, false))) return rc;
+        if ((rc = dev_alloc(c, &c->itDP, c->F, false))) return rc;
+        cd* acc = nullptr;
+        if ((rc = dev_alloc(c, &acc, 1, true))) return rc;   // one complex = two doubles
+        c->it_acc = reinterpret_cast<double*>(acc);
+    }
+    // N0 = N(u^n);  u^(1) = substep(N0) -> itA (its pressure is discarded)
+    if ((rc = launch_nonlinear(c, c->state, c->N0))) return rc;
+    if ((rc = launch_substep(c, c->N0, 1.0, nullptr, 0.0, dt, c->itA, nullptr))) return rc;
+    int k = 0;
+    double e = 0.0;
+    while (k < max_corr) {
+        // u^(k+1) = substep(c N(u^(k)) + (1 - c) N0) from (u^n, p^n) -> itB, pressure of the pass -> itP, itDP
+        if ((rc = launch_nonlinear(c, c->itA, c->N1))) return rc;
+        if ((rc = launch_substep(c, c->N1, c->p.c, c->N0, 1.0 - c->p.c, dt, c->itB, c->itP, c->itDP))) return rc;
+        if ((rc = launch_diff_norm(c, c->itA, c->itB, c->it_acc))) return rc;
+        double h[2] = {0.0, 0.0};
+        NSC_CUDA(c, cudaMemcpyAsync(h, c->it_acc, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+        NSC_CUDA(c, cudaStreamSynchronize(c->stream));
+        ++k;
+        e = h[1] > 0.0 ? sqrt(h[0] / h[1]) : 0.0;
+        for (int i = 0; i < c->nf; ++i) std::swap(c->itA[i], c->itB[i]);       // itA = newest iterate
+        if (e <= tol) break;
+    }
+    // accept: the newest iterate and the pressure of its pass become the state (pointer swaps, no copies)
+    for (int i = 0; i < c->nf; ++i) std::swap(c->state[i], c->itA[i]);
+    std::swap(c->state[4], c->itP);
+    std::swap(c->DP, c->itDP);
+    if (n_corr) *n_corr = k;
+    if (err) *err = e;
+    return NSC_OK;
 }
 
 int nsc_set_profiling(nsc_ctx* c, int on) {

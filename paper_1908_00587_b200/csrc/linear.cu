@@ -491,7 +491,8 @@ struct PoisArgs {
     cd* dst[MAXF];
     const cd* p;
     cd* p_dst;             // may be null: pressure discarded
-    cd* DP;
+    cd* DP_dst;            // D1 p of the new pressure (with p_dst)
+    const cd* DP;
     const double *D1, *rinv, *nm, *kap;
     const int* s0;
     int N_r, M1, NK, K, P, nf;
@@ -719,7 +720,7 @@ __global__ void __launch_bounds__(PBB) k_poisson_bwd_correct(PoisArgs a) {
                 if (a.copyT) a.dst[3][oc] = T;
                 if (have_p) {
                     a.p_dst[oc] = mk(fma(idt, phi.x, pr.x), fma(idt, phi.y, pr.y));
-                    a.DP[oc] = mk(fma(idt, gphi.x, dp.x), fma(idt, gphi.y, dp.y));
+                    a.DP_dst[oc] = mk(fma(idt, gphi.x, dp.x), fma(idt, gphi.y, dp.y));
                 }
             }
         }
@@ -801,6 +802,50 @@ int ensure_factors(nsc_ctx* c, double dt) {
     return NSC_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// convergence norm of the iterated corrector (R16): acc[0] += sum |b - a|^2, acc[1] += sum |b|^2
+__global__ void __launch_bounds__(256) k_diff_norm(const cd* a, const cd* b, size_t n, double* acc) {
+    double d = 0.0, s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const cd x = a[i], y = b[i];
+        const double dx = y.x - x.x, dy = y.y - x.y;
+        d = fma(dx, dx, fma(dy, dy, d));
+        s = fma(y.x, y.x, fma(y.y, y.y, s));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        d += __shfl_down_sync(0xffffffffu, d, o);
+        s += __shfl_down_sync(0xffffffffu, s, o);
+    }
+    __shared__ double sd[8], ss[8];
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) {
+        sd[w] = d;
+        ss[w] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double D = 0.0, S = 0.0;
+        for (int i = 0; i < 8; ++i) {
+            D += sd[i];
+            S += ss[i];
+        }
+        atomicAdd(acc, D);
+        atomicAdd(acc + 1, S);
+    }
+}
+
+int launch_diff_norm(nsc_ctx* c, cd* const* a, cd* const* b, double* d_acc) {
+    NSC_CUDA(c, cudaMemsetAsync(d_acc, 0, 2 * sizeof(double), c->stream));
+    for (int i = 0; i < c->nf; ++i) {
+        prof_begin(c, NSC_K_RECOMBINE);
+        k_diff_norm<<<148 * 8, 256, 0, c->stream>>>(a[i], b[i], c->F, d_acc);
+        prof_end(c);
+        NSC_CUDA(c, cudaGetLastError());
+    }
+    return NSC_OK;
+}
+
 // longest run [ja, jb) of rows whose lower (upper) width equals `width`; off = offL[ja] (offU[ja])
 static void interior_run(const BandShape& s, bool lower, int width, int& ja, int& jb, int& off) {
     const int N = (int)s.h_lo.size();
@@ -822,7 +867,7 @@ static void interior_run(const BandShape& s, bool lower, int width, int& ja, int
 }
 
 int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w1, double dt, cd* const* dst,
-                   cd* p_dst) {
+                   cd* p_dst, cd* DP_dst) {
     int rc = ensure_factors(c, dt);
     if (rc) return rc;
     const int plane = c->M1 * c->NK;
@@ -886,6 +931,7 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
         pa.p = c->state[4];
         pa.p_dst = p_dst;
         pa.DP = c->DP;
+        pa.DP_dst = DP_dst ? DP_dst : c->DP;
         pa.D1 = c->t.D1;
         pa.rinv = c->t.rinv;
         pa.nm = c->t.nm;

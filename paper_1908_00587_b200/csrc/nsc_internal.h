@@ -63,6 +63,12 @@ struct nsc_ctx {
     nsc::cd* W[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};        // sub-step work / predictor state
     nsc::cd* G = nullptr;                 // divergence / phi
     nsc::cd* DP = nullptr;                // D1 p of the state (fused linear path)
+    // iterated corrector (nsc_step_iterated), allocated on first use: ping-pong iterates, pressure of the pass
+    nsc::cd* itA[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
+    nsc::cd* itB[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
+    nsc::cd* itP = nullptr;
+    nsc::cd* itDP = nullptr;
+    double* it_acc = nullptr;
     nsc::cd* N0[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* N1[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* zbuf = nullptr;              // [JC][3 nf][N_z][MP]  z-transformed f, dz f, dr f
@@ -106,7 +112,9 @@ int ensure_factors(nsc_ctx* c, double dt);
 // one implicit sub-step from c->state with explicit term w0*E0 + w1*E1 (E1 may be null);
 // result (u, T) -> dst[0..nf-1]; new pressure -> p_dst (may be null: discarded)
 int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w1, double dt,
-                   cd* const* dst, cd* p_dst);
+                   cd* const* dst, cd* p_dst, cd* DP_dst = nullptr);
+// d_acc[0] = sum |b - a|^2, d_acc[1] = sum |b|^2 over the nf fields (device doubles)
+int launch_diff_norm(nsc_ctx* c, cd* const* a, cd* const* b, double* d_acc);
 
 // event brackets around a kernel launch (no-ops unless profiling is on); every launch site uses
 // them, and they also count the launch.

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libnsc.so")
 EXPORTS = (
     "nsc_create", "nsc_create_ex", "nsc_destroy", "nsc_set_stream", "nsc_get_grid",
     "nsc_set_state", "nsc_get_state", "nsc_set_state_host", "nsc_get_state_host",
-    "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_last_error", "nsc_device_bytes",
+    "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_step_iterated", "nsc_last_error", "nsc_device_bytes",
     "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name",
 )
 NSC_NKERN = 11
@@ -69,6 +69,7 @@ def load_library() -> C.CDLL:
     lib.nsc_nonlinear.argtypes = [vp] + [vp] * 4
     lib.nsc_substep.argtypes = [vp] + [vp] * 4 + [dbl]
     lib.nsc_step.argtypes = [vp, dbl]
+    lib.nsc_step_iterated.argtypes = [vp, dbl, dbl, i32, C.POINTER(i32), C.POINTER(dbl)]
     lib.nsc_last_error.argtypes = [vp]
     lib.nsc_last_error.restype = C.c_char_p
     lib.nsc_device_bytes.argtypes = [vp]
@@ -180,6 +181,12 @@ class Context:
 
     def substep(self, Er, Eth, Ez, ET, dt):
         self._check(self._lib.nsc_substep(self._h, _ptr(Er), _ptr(Eth), _ptr(Ez), _ptr(ET), float(dt)))
+
+    def step_iterated(self, dt, tol, max_corr):
+        """nsc_step_iterated: returns (corrector passes, last convergence norm)."""
+        k, err = C.c_int(0), C.c_double(0.0)
+        self._check(self._lib.nsc_step_iterated(self._h, dt, tol, max_corr, C.byref(k), C.byref(err)))
+        return k.value, err.value
 
     def step(self, dt):
         self._check(self._lib.nsc_step(self._h, float(dt)))

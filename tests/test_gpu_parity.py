@@ -272,3 +272,43 @@ def test_substep_uniform_grid_and_other_implicitness(torch_cuda, grid, c):
     for _ in range(2):
         ref = o.step(ref, cfg["dt"])
     assert rel_l2(got[:nf], ref[:nf]) <= TOL_STEP
+
+
+@pytest.mark.parametrize("ci,N_r,M,K,mult,amp,kmin", [(0, 24, 8, 8, 4.0, 5e-2, 2), (2, 20, 4, 8, 20.0, None, 1)])
+def test_iterated_corrector_matches_oracle(torch_cuda, ci, N_r, M, K, mult, amp, kmin):
+    """NEXT-1 (R16): nsc_step_iterated against the oracle's step_iterated -- same number of corrector
+    passes, same convergence norm, same state; one pass is bit-identical to nsc_step; a following plain
+    step still agrees (the accepted pressure and its radial derivative became the state)."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    if amp is not None:
+        cfg["amp"] = amp
+    nf = nf_of(cfg)
+    dt = mult * cfg["dt"]
+    o = oracle_of(cfg, dft="fft")
+    with _ctx(cfg) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        # one pass == nsc_step
+        ctx.set_state(*_dev(torch, st))
+        ctx.step(dt)
+        plain = ctx.state_to_host()
+        ctx.set_state(*_dev(torch, st))
+        k1, e1 = ctx.step_iterated(dt, 0.0, 1)
+        one = ctx.state_to_host()
+        assert k1 == 1 and np.isfinite(e1)
+        for a, b in zip(plain, one):
+            if a is not None:
+                np.testing.assert_array_equal(a, b)
+        # iterate to tol, then one plain step
+        tol = 1e-6
+        ctx.set_state(*_dev(torch, st))
+        k, err = ctx.step_iterated(dt, tol, 30)
+        got = ctx.state_to_host()
+        ref, k_ref, err_ref = o.step_iterated(st, dt, tol, 30)
+        assert k == k_ref and kmin <= k < 30
+        assert abs(err - err_ref) <= 1e-3 * err_ref + 1e-15
+        assert rel_l2(got[:nf], ref[:nf]) <= TOL_STEP
+        ctx.step(dt)
+        got2 = ctx.state_to_host()
+    ref2 = o.step(ref, dt)
+    assert rel_l2(got2[:nf], ref2[:nf]) <= TOL_STEP
