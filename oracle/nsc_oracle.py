@@ -408,6 +408,41 @@ class Oracle:
                 break
         return cur, k, err
 
+    # ---------------------------------------------------------------- NEXT-3: diagnostics
+    def nusselt(self, state):
+        """Wall diagnostics of PAPER.md:100-108 (Fig. 3a plots Nu_i): transfer at a wall normalised by that of
+        the basic state at the same parameters, from the mean mode (0,0) only (theta, z averages).
+          heat  : Nu = d_r T^(0,0) / d_r T_b,        T_b = ln(r / r_o) / ln(eta) - 1/2  =>  d_r T_b = 1 / (r ln eta)
+          torque: Nu_w = [r^3 d_r(u_theta / r)] / [r^3 d_r(V / r)],  V = A r + B / r   =>  r^3 d_r(V / r) = -2 B
+        (u_r = 0 at the walls, so the convective part of both fluxes vanishes there).  d_r = the 9-point D1 row
+        of the wall node.  Returns (Nu_i, Nu_o, Nu_w_i, Nu_w_o); the heat entries are nan without temperature."""
+        p = self.p
+        ur, ut, uz, T, pr = state
+        r = self.r
+        K = p.K
+        eta = p.eta
+        B = eta * (p.Re_i - eta * p.Re_o) / ((1 - eta) * (1 - eta ** 2))
+        out = []
+        for j in (0, p.N_r - 1):
+            if p.heated:
+                dT = float((self.D1[j] @ T[:, 0, K]).real)
+                out.append(dT * r[j] * np.log(eta))
+            else:
+                out.append(float("nan"))
+        for j in (0, p.N_r - 1):
+            v = ut[:, 0, K].real
+            dw = (self.D1[j] @ v) / r[j] - v[j] / r[j] ** 2
+            out.append(float(r[j] ** 3 * dw / (-2.0 * B)) if B != 0.0 else float("nan"))
+        return tuple(out)
+
+    def probe(self, f, j, theta, z):
+        """Value of the physical field of spectral coefficients ``f`` at radial node j and the point (theta, z)
+        (Fig. 3b: u_theta at a fixed probe location): the series of O3 at an arbitrary point,
+        Re sum_k f(0,k) e^{i kappa z} + 2 Re sum_{m>=1} sum_k f(m,k) e^{i (n theta + kappa z)}."""
+        ph = np.exp(1j * (self.n[:, None] * theta + self.kappa[None, :] * z))
+        t = f[j] * ph
+        return float(t[0].sum().real + 2.0 * t[1:].sum().real)
+
     # ---------------------------------------------------------------- basic states
     def zeros(self):
         p = self.p

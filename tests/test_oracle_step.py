@@ -291,3 +291,64 @@ def test_iterated_corrector_leaves_couette_flow_alone():
     out, k, err = o.step_iterated(base, 1e-2, tol=1e-12, max_corr=5)
     assert k == 1 and err <= 1e-12
     assert rel_l2(out[:3], base[:3]) <= 1e-13
+
+
+# ---------------------------------------------------------------- NEXT-3: diagnostics
+def test_nusselt_numbers_are_one_in_the_basic_state():
+    """Nu_i is normalised by the basic state, so it is 1 there -- at both walls, for the heat
+    flux and for the torque, up to the truncation error of the discrete profiles (falls with N_r)."""
+    from paper_1908_00587_b200 import synth
+    from helpers import oracle_of
+    errs = []
+    for N_r in (24, 48):
+        cfg = synth.scaled_config(2, N_r=N_r, M=4, K=4)          # heated, both cylinders rotating
+        o = oracle_of(cfg, dft="fft")
+        nu = np.array(o.nusselt(o.base_state_discrete()))
+        errs.append(np.max(np.abs(nu - 1.0)))
+    assert errs[0] < 1e-5 and errs[1] < 1e-8 and errs[1] < errs[0]
+    cfg = synth.scaled_config(0, N_r=24, M=4, K=4)               # no temperature: heat entries are nan
+    o = oracle_of(cfg, dft="fft")
+    nu = o.nusselt(o.base_state_discrete())
+    assert np.isnan(nu[0]) and np.isnan(nu[1]) and abs(nu[2] - 1) < 1e-5 and abs(nu[3] - 1) < 1e-5
+
+
+def test_nusselt_of_a_manufactured_profile():
+    """A profile with a known wall derivative: T = T_b + a (r - r_i)^2 (r_o - r) adds nothing at the inner wall
+    and a (r_o - r_i)^2 * (-1) at the outer one; u_theta = V + b (r - r_i)(r_o - r) changes the torque by the
+    closed-form amount (polynomials of degree <= 8: the 9-point rows are exact)."""
+    from paper_1908_00587_b200 import synth
+    from helpers import oracle_of
+    cfg = synth.scaled_config(2, N_r=32, M=4, K=4)
+    o = oracle_of(cfg, dft="fft")
+    st = o.base_state_discrete()
+    base = np.array(o.nusselt(st))
+    r, K, eta = o.r, cfg["K"], cfg["eta"]
+    ri, ro = r[0], r[-1]
+    a, b = 0.3, 7.0
+    st[3][:, 0, K] += a * (r - ri) ** 2 * (ro - r)
+    st[1][:, 0, K] += b * (r - ri) * (ro - r)
+    nu = np.array(o.nusselt(st))
+    B = eta * (cfg["Re_i"] - eta * cfg["Re_o"]) / ((1 - eta) * (1 - eta ** 2))
+    want = base + np.array([0.0, -a * (ro - ri) ** 2 * ro * np.log(eta),
+                            ri ** 3 * (b * (ro - ri) / ri) / (-2 * B), ro ** 3 * (-b * (ro - ri) / ro) / (-2 * B)])
+    np.testing.assert_allclose(nu, want, rtol=0, atol=1e-9)
+
+
+def test_probe_equals_the_transform_on_grid_points_and_a_single_mode_elsewhere():
+    from paper_1908_00587_b200 import synth
+    from helpers import oracle_of
+    cfg = synth.scaled_config(1, N_r=12, M=4, K=4)
+    o = oracle_of(cfg, dft="naive")
+    st = synth.make_state(cfg, o.r)
+    phys = o.to_physical(st[1])                                  # [N_r, N_theta, N_z]
+    Nt, Nz = phys.shape[1], phys.shape[2]
+    for (j, a, b) in [(0, 0, 0), (5, 3, 7), (11, Nt - 1, Nz - 1)]:
+        theta = 2 * np.pi * a / (Nt * cfg["k_theta0"])
+        z = 2 * np.pi * b / (Nz * cfg["alpha"])
+        assert abs(o.probe(st[1], j, theta, z) - phys[j, a, b]) <= 1e-12 * np.max(np.abs(phys))
+    f = o.zeros()
+    f[:, 2, cfg["K"] + 3] = 1.5 - 0.5j                           # single mode (m, k) = (2, 3)
+    theta, z = 0.37, 1.1
+    n, kap = 2 * cfg["k_theta0"], 3 * cfg["alpha"]
+    want = 2 * ((1.5 - 0.5j) * np.exp(1j * (n * theta + kap * z))).real
+    assert abs(o.probe(f, 4, theta, z) - want) <= 1e-13
