@@ -126,6 +126,18 @@ int nsc_step(nsc_ctx* ctx, double dt);
  * (2 n_f + 2) more field-sized buffers. */
 int nsc_step_iterated(nsc_ctx* ctx, double dt, double tol, int max_corr, int* n_corr, double* err);
 
+/* Wall diagnostics of the current state (Fig. 3a): transfer at a wall
+ * normalised by that of the basic state at the same parameters, from the mean mode (0,0):
+ *   h_out[0], h_out[1]  heat-flux Nusselt number at the inner / outer wall, d_r T r ln(eta)  (nan if Ra = 0)
+ *   h_out[2], h_out[3]  torque Nusselt number, r^3 d_r(u_theta / r) / (-2 B), B of the Couette profile (nan if B = 0)
+ * d_r is the 9-point row of the wall node.  h_out: HOST array of 4 doubles.  Synchronises the stream. */
+int nsc_nusselt(nsc_ctx* ctx, double* h_out);
+
+/* Value of a physical field at radial node j and the point (theta, z) (Fig. 3b: u_theta at a
+ * fixed probe location): the Fourier series of the state evaluated there.  field: 0 u_r, 1 u_theta, 2 u_z, 3 T,
+ * 4 p.  *h_value: HOST double.  Synchronises the stream. */
+int nsc_probe(nsc_ctx* ctx, int field, int j, double theta, double z, double* h_value);
+
 /* Text of the last error of this context ("" if none); valid until the next call on ctx.
  * With ctx == NULL: the text of the last failed nsc_create on this thread. */
 const char* nsc_last_error(const nsc_ctx* ctx);
@@ -148,7 +160,7 @@ enum {
     NSC_K_RHS = 3,       /* L1 + L2 (k_rhs_fwd): right-hand sides + forward substitution, marching up   */
     NSC_K_HELMHOLTZ = 4, /* L2 + L3 (k_bwd_div): back substitution, recombination, divergence, down     */
     NSC_K_RECOMBINE = 5, /* k_diff_norm: convergence norm of the iterated corrector (nsc_step_iterated)  */
-    NSC_K_DIV = 6,       /* (unused: fused into k_bwd_div)                                               */
+    NSC_K_DIV = 6,       /* k_nusselt / k_probe: diagnostics (nsc_nusselt, nsc_probe)                    */
     NSC_K_POISSON = 7,   /* L4 (k_poisson_fwd): forward substitution of the pressure system, up          */
     NSC_K_CORRECT = 8,   /* L4 + L5 (k_poisson_bwd_correct): back substitution + correction, down        */
     NSC_K_FACTOR = 9,    /* set-up: banded LU of the per-mode matrices (once per dt)                 */

@@ -68,7 +68,7 @@ void prof_end(nsc_ctx* c) {
 }
 
 static const char* kKernelNames[NSC_NKERN] = {"k_zinv", "k_theta", "k_zfwd", "k_rhs_fwd", "k_bwd_div",
-                                              "k_diff_norm", "(unused)", "k_poisson_fwd", "k_poisson_bwd_correct",
+                                              "k_diff_norm", "k_nusselt / k_probe", "k_poisson_fwd", "k_poisson_bwd_correct",
                                               "k_factor", "k_dr"};
 
 static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
@@ -361,6 +361,38 @@ int nsc_step_iterated(nsc_ctx* c, double dt, double tol, int max_corr, int* n_co
     std::swap(c->DP, c->itDP);
     if (n_corr) *n_corr = k;
     if (err) *err = e;
+    return NSC_OK;
+}
+
+static int diag_scratch(nsc_ctx* c) {
+    if (c->diag) return NSC_OK;
+    cd* p = nullptr;
+    int rc = dev_alloc(c, &p, 2, true);                  // two complex = four doubles
+    if (!rc) c->diag = reinterpret_cast<double*>(p);
+    return rc;
+}
+
+int nsc_nusselt(nsc_ctx* c, double* h_out) {
+    if (!c || !h_out) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_nusselt before nsc_set_state");
+    int rc = diag_scratch(c);
+    if (rc) return rc;
+    if ((rc = launch_nusselt(c, c->diag))) return rc;
+    NSC_CUDA(c, cudaMemcpyAsync(h_out, c->diag, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    NSC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NSC_OK;
+}
+
+int nsc_probe(nsc_ctx* c, int field, int j, double theta, double z, double* h_value) {
+    if (!c || !h_value) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_probe before nsc_set_state");
+    if (field < 0 || field > 4 || (field == 3 && !c->heated) || j < 0 || j >= c->N_r)
+        return fail(c, NSC_EINVAL, "nsc_probe: field must be 0..4 (3 only with temperature) and 0 <= j < N_r");
+    int rc = diag_scratch(c);
+    if (rc) return rc;
+    if ((rc = launch_probe(c, c->state[field], j, theta, z, c->diag))) return rc;
+    NSC_CUDA(c, cudaMemcpyAsync(h_value, c->diag, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    NSC_CUDA(c, cudaStreamSynchronize(c->stream));
     return NSC_OK;
 }
 

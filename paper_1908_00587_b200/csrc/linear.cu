@@ -846,6 +846,78 @@ int launch_diff_norm(nsc_ctx* c, cd* const* a, cd* const* b, double* d_acc) {
     return NSC_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// NEXT-3 diagnostics.  k_nusselt: out[0..1] heat, out[2..3] torque Nusselt numbers at the
+// inner / outer wall from the mean mode (0,0): Nu = d_r T r ln(eta);  Nu_w = r^3 d_r(u_theta / r) / (-2 B).
+__global__ void k_nusselt(const cd* ut, const cd* T, const double* D1, const int* s0, const double* rinv, int N_r,
+                          size_t plane, size_t col00, double ln_eta, double B, double* out) {
+    const int t = threadIdx.x;
+    if (t >= 4) return;
+    const int j = (t & 1) ? N_r - 1 : 0;
+    const cd* f = (t < 2) ? T : ut;
+    double v = nan("");
+    if (f) {
+        double d = 0.0;
+        for (int l = 0; l < NPT; ++l) d = fma(D1[j * NPT + l], f[(size_t)(s0[j] + l) * plane + col00].x, d);
+        const double ri = rinv[j], r = 1.0 / ri;
+        if (t < 2) {
+            v = d * r * ln_eta;
+        } else if (B != 0.0) {
+            const double dw = d * ri - f[(size_t)j * plane + col00].x * ri * ri;
+            v = r * r * r * dw / (-2.0 * B);
+        }
+    }
+    out[t] = v;
+}
+
+// k_probe: acc += Re sum_k f(0,k) e^{i kappa z} + 2 Re sum_{m>=1,k} f(m,k) e^{i(n theta + kappa z)} at one radial node
+__global__ void __launch_bounds__(256) k_probe(const cd* fj, const double* nm, const double* kap, int M1, int NK,
+                                               double theta, double z, double* acc) {
+    double s = 0.0;
+    const int n = M1 * NK;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+        const int m = e / NK, kk = e % NK;
+        double sn, cs;
+        sincos(nm[m] * theta + kap[kk] * z, &sn, &cs);
+        const cd v = fj[e];
+        const double re = v.x * cs - v.y * sn;
+        s += (m == 0) ? re : 2.0 * re;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    __shared__ double sh[8];
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double S = 0.0;
+        for (int i = 0; i < 8; ++i) S += sh[i];
+        atomicAdd(acc, S);
+    }
+}
+
+int launch_nusselt(nsc_ctx* c, double* d_out) {
+    const double eta = c->p.eta;
+    const double B = eta * (c->p.Re_i - eta * c->p.Re_o) / ((1.0 - eta) * (1.0 - eta * eta));
+    prof_begin(c, NSC_K_DIV);
+    k_nusselt<<<1, 32, 0, c->stream>>>(c->state[1], c->heated ? c->state[3] : nullptr, c->t.D1, c->t.s0, c->t.rinv,
+                                        c->N_r, (size_t)c->M1 * c->NK, (size_t)c->K, log(eta), B, d_out);
+    prof_end(c);
+    NSC_CUDA(c, cudaGetLastError());
+    return NSC_OK;
+}
+
+int launch_probe(nsc_ctx* c, const cd* field, int j, double theta, double z, double* d_acc) {
+    NSC_CUDA(c, cudaMemsetAsync(d_acc, 0, sizeof(double), c->stream));
+    const int n = c->M1 * c->NK;
+    int blocks = (n + 255) / 256;
+    if (blocks > 592) blocks = 592;
+    prof_begin(c, NSC_K_DIV);
+    k_probe<<<blocks, 256, 0, c->stream>>>(field + (size_t)j * n, c->t.nm, c->t.kap, c->M1, c->NK, theta, z, d_acc);
+    prof_end(c);
+    NSC_CUDA(c, cudaGetLastError());
+    return NSC_OK;
+}
+
 // longest run [ja, jb) of rows whose lower (upper) width equals `width`; off = offL[ja] (offU[ja])
 static void interior_run(const BandShape& s, bool lower, int width, int& ja, int& jb, int& off) {
     const int N = (int)s.h_lo.size();

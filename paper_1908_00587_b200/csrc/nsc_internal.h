@@ -69,6 +69,7 @@ struct nsc_ctx {
     nsc::cd* itP = nullptr;
     nsc::cd* itDP = nullptr;
     double* it_acc = nullptr;
+    double* diag = nullptr;               // device scratch of the diagnostics (4 doubles)
     nsc::cd* N0[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* N1[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* zbuf = nullptr;              // [JC][3 nf][N_z][MP]  z-transformed f, dz f, dr f
@@ -115,6 +116,9 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
                    cd* const* dst, cd* p_dst, cd* DP_dst = nullptr);
 // d_acc[0] = sum |b - a|^2, d_acc[1] = sum |b|^2 over the nf fields (device doubles)
 int launch_diff_norm(nsc_ctx* c, cd* const* a, cd* const* b, double* d_acc);
+// diagnostics (NEXT-3): d_out[4] = Nu_i, Nu_o (heat), Nu_w_i, Nu_w_o (torque); d_acc = field value at (r_j, theta, z)
+int launch_nusselt(nsc_ctx* c, double* d_out);
+int launch_probe(nsc_ctx* c, const cd* field, int j, double theta, double z, double* d_acc);
 
 // event brackets around a kernel launch (no-ops unless profiling is on); every launch site uses
 // them, and they also count the launch.

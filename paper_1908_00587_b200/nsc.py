@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libnsc.so")
 EXPORTS = (
     "nsc_create", "nsc_create_ex", "nsc_destroy", "nsc_set_stream", "nsc_get_grid",
     "nsc_set_state", "nsc_get_state", "nsc_set_state_host", "nsc_get_state_host",
-    "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_step_iterated", "nsc_last_error", "nsc_device_bytes",
+    "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_step_iterated", "nsc_nusselt", "nsc_probe", "nsc_last_error", "nsc_device_bytes",
     "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name",
 )
 NSC_NKERN = 11
@@ -69,6 +69,8 @@ def load_library() -> C.CDLL:
     lib.nsc_nonlinear.argtypes = [vp] + [vp] * 4
     lib.nsc_substep.argtypes = [vp] + [vp] * 4 + [dbl]
     lib.nsc_step.argtypes = [vp, dbl]
+    lib.nsc_nusselt.argtypes = [vp, C.POINTER(dbl)]
+    lib.nsc_probe.argtypes = [vp, i32, i32, dbl, dbl, C.POINTER(dbl)]
     lib.nsc_step_iterated.argtypes = [vp, dbl, dbl, i32, C.POINTER(i32), C.POINTER(dbl)]
     lib.nsc_last_error.argtypes = [vp]
     lib.nsc_last_error.restype = C.c_char_p
@@ -181,6 +183,18 @@ class Context:
 
     def substep(self, Er, Eth, Ez, ET, dt):
         self._check(self._lib.nsc_substep(self._h, _ptr(Er), _ptr(Eth), _ptr(Ez), _ptr(ET), float(dt)))
+
+    def nusselt(self):
+        """nsc_nusselt: (Nu_i, Nu_o, Nu_w_i, Nu_w_o) of the current state."""
+        out = (C.c_double * 4)()
+        self._check(self._lib.nsc_nusselt(self._h, out))
+        return tuple(out)
+
+    def probe(self, field, j, theta, z):
+        """nsc_probe: the physical field ``field`` (0 u_r, 1 u_theta, 2 u_z, 3 T, 4 p) at (r_j, theta, z)."""
+        v = C.c_double(0.0)
+        self._check(self._lib.nsc_probe(self._h, field, j, theta, z, C.byref(v)))
+        return v.value
 
     def step_iterated(self, dt, tol, max_corr):
         """nsc_step_iterated: returns (corrector passes, last convergence norm)."""

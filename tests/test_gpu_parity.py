@@ -312,3 +312,30 @@ def test_iterated_corrector_matches_oracle(torch_cuda, ci, N_r, M, K, mult, amp,
         got2 = ctx.state_to_host()
     ref2 = o.step(ref, dt)
     assert rel_l2(got2[:nf], ref2[:nf]) <= TOL_STEP
+
+
+@pytest.mark.parametrize("ci,N_r,M,K", [(2, 24, 8, 8), (0, 20, 4, 8)])
+def test_diagnostics_match_oracle(torch_cuda, ci, N_r, M, K):
+    """NEXT-3: nsc_nusselt and nsc_probe against the oracle's nusselt / probe, before and after steps."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    nf = nf_of(cfg)
+    o = oracle_of(cfg, dft="fft")
+    with _ctx(cfg) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        for it in range(2):
+            got = np.array(ctx.nusselt())
+            ref = np.array(o.nusselt(st))
+            assert np.array_equal(np.isnan(got), np.isnan(ref))
+            np.testing.assert_allclose(got[~np.isnan(ref)], ref[~np.isnan(ref)], rtol=1e-11, atol=1e-12)
+            for field, j, th, z in [(1, N_r // 2, 0.3, 0.7), (0, 1, 1.9, 0.05), (2, N_r - 2, 0.0, 0.0), (4, 3, 2.5, 1.0)]:
+                ref_v = o.probe(st[field], j, th, z)
+                scale = max(1.0, np.abs(st[field][j]).sum())
+                assert abs(ctx.probe(field, j, th, z) - ref_v) <= 1e-12 * scale
+            if nf == 4:
+                assert abs(ctx.probe(3, 2, 0.4, 0.4) - o.probe(st[3], 2, 0.4, 0.4)) <= 1e-12
+            ctx.step(cfg["dt"])
+            st = o.step(st, cfg["dt"])
+        with pytest.raises(Exception):
+            ctx.probe(3 if nf == 3 else 5, 0, 0.0, 0.0)
