@@ -339,3 +339,22 @@ def test_diagnostics_match_oracle(torch_cuda, ci, N_r, M, K):
             st = o.step(st, cfg["dt"])
         with pytest.raises(Exception):
             ctx.probe(3 if nf == 3 else 5, 0, 0.0, 0.0)
+
+
+@pytest.mark.parametrize("ci,N_r,M,K,chunk", [(1, 10, 8, 256, 4), (3, 12, 256, 8, 5), (3, 11, 256, 256, 3)])
+def test_nonlinear_length_768_in_several_radial_chunks(torch_cuda, ci, N_r, M, K, chunk):
+    """The multi-chunk form of the length-768 pipeline (spectral k_dr + three z transforms per line, used when
+    the work arrays of the whole radius do not fit) against the oracle, and against the single-chunk form."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    o = oracle_of(cfg, dft="fft")
+    res = []
+    for rc in (chunk, 0):
+        with _ctx(cfg, radial_chunk=rc) as ctx:
+            st = synth.make_state(cfg, ctx.grid())
+            ctx.set_state(*_dev(torch, st))
+            res.append(ctx.nonlinear_to_host())
+    ref = o.nonlinear(*st[:3])
+    assert rel_l2(res[0], ref) <= TOL_N
+    assert rel_l2(res[1], ref) <= TOL_N
+    assert rel_l2(res[0], res[1]) <= 1e-13
