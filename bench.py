@@ -270,7 +270,8 @@ def run_ours(args, cfg, rank, world, local_rank):
     s = sizes(cfg)
     nf, F = s["nf"], s["F"]
     dt = cfg["dt"]
-    stream = torch.cuda.current_stream()
+    stream = torch.cuda.Stream()            # a non-default stream: nsc_step replays its CUDA graph on it
+    torch.cuda.set_stream(stream)
 
     def barrier():
         torch.cuda.synchronize()

@@ -159,6 +159,7 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
         if (!rc) rc = dev_alloc(c, &c->zbuf, (size_t)3 * c->nf * c->JC * c->Nz * c->MP, true);
         if (!rc) rc = dev_alloc(c, &c->tbuf, (size_t)c->nf * c->JC * c->Nz * c->MP, true);
     }
+    if (const char* ev = getenv("NSC_GRAPH")) c->use_graph = atoi(ev) != 0;
     if (const char* ev = getenv("NSC_LIN_SLICES")) c->n_slices = atoi(ev);
     if (c->n_slices < 1) c->n_slices = 1;
     if (c->n_slices > NSC_MAX_SLICES) c->n_slices = NSC_MAX_SLICES;
@@ -207,6 +208,7 @@ int nsc_destroy(nsc_ctx* c) {
         cudaEventDestroy(r.b);
     }
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     for (cudaStream_t s : c->slice_stream)
         if (s) cudaStreamDestroy(s);
     for (cudaEvent_t e : c->slice_ev)
@@ -307,10 +309,8 @@ int nsc_substep(nsc_ctx* c, const void* Er, const void* Eth, const void* Ez, con
     return launch_substep(c, E, 1.0, nullptr, 0.0, dt, c->state, c->state[4]);
 }
 
-int nsc_step(nsc_ctx* c, double dt) {
-    if (!c) return NSC_EINVAL;
-    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_step before nsc_set_state");
-    if (!(dt > 0.0)) return fail(c, NSC_EINVAL, "nsc_step: dt must be > 0");
+// the kernel sequence of one step (R10)
+static int step_body(nsc_ctx* c, double dt) {
     int rc;
     // N0 = N(u^n);  u^1 = substep(N0) -> W (its pressure is discarded)
     if ((rc = launch_nonlinear(c, c->state, c->N0))) return rc;
@@ -318,6 +318,55 @@ int nsc_step(nsc_ctx* c, double dt) {
     // N1 = N(u^1);  u^{n+1} = substep(c N1 + (1 - c) N0) from (u^n, p^n), in place
     if ((rc = launch_nonlinear(c, c->W, c->N1))) return rc;
     return launch_substep(c, c->N1, c->p.c, c->N0, 1.0 - c->p.c, dt, c->state, c->state[4]);
+}
+
+static void drop_graph(nsc_ctx* c) {
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    c->graph_exec = nullptr;
+}
+
+int nsc_step(nsc_ctx* c, double dt) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_step before nsc_set_state");
+    if (!(dt > 0.0)) return fail(c, NSC_EINVAL, "nsc_step: dt must be > 0");
+    // The ~44 launches of a step are captured once per (dt, stream, buffer generation) into a CUDA graph and
+    // replayed: small configurations are launch-bound.  With per-kernel profiling on (event brackets), or if
+    // capture is not possible, the kernels are launched one by one.
+    if (c->use_graph && !c->profiling) {
+        const bool stale = !c->graph_exec || c->graph_dt != dt || c->graph_stream != c->stream || c->graph_gen != c->ptr_gen;
+        if (stale) {
+            drop_graph(c);
+            int rc = ensure_factors(c, dt);             // set-up kernels stay outside the graph
+            if (rc) return rc;
+            cudaGraph_t g = nullptr;
+            const long long l0 = c->launches;
+            if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                rc = step_body(c, dt);
+                const cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+                if (rc == NSC_OK && e == cudaSuccess && g && cudaGraphInstantiate(&c->graph_exec, g, 0) == cudaSuccess) {
+                    c->graph_dt = dt;
+                    c->graph_stream = c->stream;
+                    c->graph_gen = c->ptr_gen;
+                    c->graph_launches = c->launches - l0;
+                } else {
+                    c->graph_exec = nullptr;
+                    c->use_graph = false;                // fall back to plain launches for good
+                }
+                if (g) cudaGraphDestroy(g);
+                cudaGetLastError();
+            } else {
+                cudaGetLastError();
+                c->use_graph = false;
+            }
+            c->launches = l0;
+        }
+        if (c->graph_exec) {
+            NSC_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
+            c->launches += c->graph_launches;
+            return NSC_OK;
+        }
+    }
+    return step_body(c, dt);
 }
 
 int nsc_step_iterated(nsc_ctx* c, double dt, double tol, int max_corr, int* n_corr, double* err) {
@@ -359,6 +408,7 @@ int nsc_step_iterated(nsc_ctx* c, double dt, double tol, int max_corr, int* n_co
     for (int i = 0; i < c->nf; ++i) std::swap(c->state[i], c->itA[i]);
     std::swap(c->state[4], c->itP);
     std::swap(c->DP, c->itDP);
+    c->ptr_gen += 1;                                     // a captured step graph holds the old pointers
     if (n_corr) *n_corr = k;
     if (err) *err = e;
     return NSC_OK;

@@ -83,6 +83,12 @@ struct nsc_ctx {
     bool facT_shared = false;             // T shares the u_z factors (Pr == 1)
     double fac_dt = 0.0;                  // dt the Helmholtz factors were built for (0: none)
     bool facP_ready = false;
+    // CUDA graph of one nsc_step (NSC_GRAPH=0 disables)
+    bool use_graph = true;
+    cudaGraphExec_t graph_exec = nullptr;
+    double graph_dt = 0.0;
+    cudaStream_t graph_stream = nullptr;
+    long long graph_gen = -1, ptr_gen = 0, graph_launches = 0;
     int n_slices = 2;                                 // mode slices of the linear stage (NSC_LIN_SLICES overrides)
     cudaStream_t slice_stream[NSC_MAX_SLICES] = {};   // their streams
     cudaEvent_t slice_ev[NSC_MAX_SLICES + 1] = {};    // [0] fork, [1 + s] join of slice s

@@ -396,3 +396,35 @@ def test_full_size_cfg5_sampled(torch_cuda):
     err_s = rel_l2(got_s, ref_s[:4])
     print("cfg 5 sampled: sub-step rel-L2", err_s)
     assert err_s <= TOL_STEP
+
+
+def test_step_graph_replay_equals_plain_launches(torch_cuda):
+    """On a non-default stream nsc_step captures its kernel sequence into a CUDA graph and replays it; on the
+    legacy default stream (no capture possible) it launches kernel by kernel.  Same bits, same launch count;
+    a change of dt or an nsc_step_iterated in between (buffer swap) re-captures."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(1, N_r=20, M=8, K=8)
+    dt = cfg["dt"]
+    res, counts = [], []
+    for side in (False, True):
+        with _ctx(cfg) as ctx:
+            s = torch.cuda.Stream() if side else None
+            if side:
+                ctx.set_stream(s)
+            st = synth.make_state(cfg, ctx.grid())
+            ctx.set_state(*_dev(torch, st))
+            torch.cuda.synchronize()
+            n0 = ctx.launch_count()
+            for _ in range(3):
+                ctx.step(dt)
+            ctx.step(0.5 * dt)
+            ctx.step_iterated(dt, 0.0, 2)
+            for _ in range(2):
+                ctx.step(dt)
+            torch.cuda.synchronize()
+            counts.append(ctx.launch_count() - n0)
+            res.append(ctx.state_to_host())
+    assert counts[0] == counts[1]
+    for a, b in zip(*res):
+        if a is not None:
+            np.testing.assert_array_equal(a, b)
