@@ -30,6 +30,14 @@ tests/test_oracle_transforms.py) so that the large configurations finish.
 
 Linear solves are dense Gaussian elimination with partial pivoting after row
 equilibration (LAPACK ``gesv`` through ``numpy.linalg.solve`` on row-scaled matrices).
+``solve="banded"`` is the second backend BASELINE.json north_star allows ("dense or banded
+Gaussian elimination"): the same matrices held by diagonals and eliminated row by row without
+pivoting, vectorised over the Fourier modes, and the radial operators applied through their
+9-point rows instead of dense matrices.  It is pinned to the dense backend
+(tests/test_oracle_banded.py) and exists so that 20-step runs at the large configurations
+finish; plain numpy throughout, so it also runs in ``real=numpy.longdouble`` (SURVEY.md 8(c):
+"oracle(double) vs oracle(long double) after 20 steps is reported as the floor"), where the
+tables are kept in extended precision instead of being rounded to double.
 
 Parity unpinned (defined by the algorithm only): the pressure field,
 the O(dt^2) tangential wall slip, and the aliased extreme modes |k| = K, m = M.
@@ -142,11 +150,11 @@ def fd_tables(r_ld, npt: int = 9):
     return D1, D2
 
 
-def roots_of_unity(N: int):
+def roots_of_unity(N: int, real=np.float64):
     """exp(2 pi i t / N), t = 0..N-1, evaluated in long double, rounded once (O3)."""
     t = np.arange(N, dtype=LD)
     ang = 2 * _pi_ld() * t / N
-    return np.cos(ang).astype(np.float64) + 1j * np.sin(ang).astype(np.float64)
+    return np.cos(ang).astype(real) + 1j * np.sin(ang).astype(real)
 
 
 # --------------------------------------------------------------------------------------
@@ -155,9 +163,16 @@ def roots_of_unity(N: int):
 class Oracle:
     """One Taylor-Couette configuration; methods follow O3..O8 in SURVEY.md 8(c)."""
 
-    def __init__(self, p: Params, dft: str = "naive"):
+    def __init__(self, p: Params, dft: str = "naive", solve: str = "dense", real=np.float64):
+        if solve not in ("dense", "banded"):
+            raise ValueError("solve must be 'dense' or 'banded'")
+        if real is not np.float64 and solve != "banded":
+            raise ValueError("extended precision needs solve='banded' (LAPACK is double only)")
         self.p = p
         self.dft = dft
+        self.solve = solve
+        self.real = real
+        self.cplx = np.result_type(real, np.complex64)       # complex128 / clongdouble
         N_r = p.N_r
         r_ld = radial_grid(N_r, p.eta, p.grid, dtype=LD)
         D1, D2 = fd_tables(r_ld)
@@ -167,7 +182,7 @@ class Oracle:
         Gt[0, :] = 0
         Gt[-1, :] = 0
         Q = (D1 + np.diag(inv_r)) @ Gt                       # (D1 + 1/r) G~, product in LD
-        f64 = np.float64
+        f64 = real
         self.r = r_ld.astype(f64)
         self.D1, self.D2 = D1.astype(f64), D2.astype(f64)
         self.L0, self.Gt, self.Q = L0.astype(f64), Gt.astype(f64), Q.astype(f64)
@@ -175,15 +190,21 @@ class Oracle:
         self.n = (np.arange(p.M + 1) * p.k_theta0).astype(f64)          # [M+1]
         self.kappa = (np.arange(-p.K, p.K + 1) * p.alpha).astype(f64)   # [2K+1]
         # O3 root tables, indexed by (m*a mod N_theta), (k*b mod N_z)
-        wt = roots_of_unity(p.n_theta)
-        wz = roots_of_unity(p.n_z)
+        wt = roots_of_unity(p.n_theta, real)
+        wz = roots_of_unity(p.n_z, real)
         m = np.arange(p.M + 1)[:, None]
         a = np.arange(p.n_theta)[None, :]
         k = np.arange(-p.K, p.K + 1)[:, None]
         b = np.arange(p.n_z)[None, :]
         self.Et = wt[(m * a) % p.n_theta]                    # [M+1, N_theta]
         self.Ez = wz[(k * b) % p.n_z]                        # [2K+1, N_z]
-        self.cm = np.where(np.arange(p.M + 1) == 0, 1.0, 2.0)
+        self.cm = np.where(np.arange(p.M + 1) == 0, 1.0, 2.0).astype(f64)
+        # band form of the radial operators (solve="banded"): row j of D1 / L0 on its stencil S(j)
+        self.s0 = np.array([stencil_start(j, N_r) for j in range(N_r)])
+        cols = self.s0[:, None] + np.arange(9)[None, :]
+        rows = np.arange(N_r)[:, None]
+        self.D1_rows = self.D1[rows, cols]                   # [N_r, 9]
+        self.L0_rows = self.L0[rows, cols]
 
     # ---------------------------------------------------------------- O3 transforms
     def to_physical(self, fh):
@@ -192,7 +213,7 @@ class Oracle:
         fh: [..., M+1, 2K+1] -> real [..., N_theta, N_z]."""
         p = self.p
         if self.dft == "fft":
-            pad = np.zeros(fh.shape[:-2] + (p.n_theta // 2 + 1, p.n_z), complex)
+            pad = np.zeros(fh.shape[:-2] + (p.n_theta // 2 + 1, p.n_z), self.cplx)
             kk = np.arange(-p.K, p.K + 1) % p.n_z
             pad[..., :p.M + 1, kk] = fh
             half = np.fft.ifft(pad, axis=-1) * p.n_z
@@ -214,8 +235,18 @@ class Oracle:
         return (t @ np.conj(self.Ez).T) / (p.n_theta * p.n_z)
 
     # ---------------------------------------------------------------- O5 operators
+    def _rows9(self, rows9, f, js=None):
+        """sum_{l in S(j)} rows9[j, l - s0(j)] f_l written out over the nine stencil nodes (banded backend)."""
+        js = np.arange(self.p.N_r) if js is None else np.asarray(js)
+        out = np.zeros((len(js),) + f.shape[1:], np.result_type(f.dtype, rows9.dtype))
+        for l in range(9):
+            out += rows9[js, l][:, None, None] * f[self.s0[js] + l]
+        return out
+
     def d_r(self, f):
         """Radial derivative: sum_{l in S(j)} D1[j,l] f_l (N1)."""
+        if self.solve == "banded":
+            return self._rows9(self.D1_rows, f)
         return np.einsum("jl,lmk->jmk", self.D1, f)
 
     def lap(self, f, shift: int):
@@ -223,6 +254,8 @@ class Oracle:
         shift = +-1: L_+- acting on u_+- = u_r +- i u_theta (O5)."""
         q = ((self.n[None, :, None] + shift) ** 2 / self.r[:, None, None] ** 2
              + self.kappa[None, None, :] ** 2)
+        if self.solve == "banded":
+            return self._rows9(self.L0_rows, f) - q * f
         return np.einsum("jl,lmk->jmk", self.L0, f) - q * f
 
     def divergence(self, ur, ut, uz):
@@ -247,7 +280,8 @@ class Oracle:
         for f in fields:
             fj = f[js]
             ph.append(self.to_physical(fj))
-            d_r.append(self.to_physical(np.einsum("jl,lmk->jmk", self.D1[js], f)))
+            d_r.append(self.to_physical(self._rows9(self.D1_rows, f, js) if self.solve == "banded"
+                                        else np.einsum("jl,lmk->jmk", self.D1[js], f)))
             d_t.append(self.to_physical(i_n * fj))
             d_z.append(self.to_physical(i_k * fj))
         Ur, Ut, Uz = ph[0], ph[1], ph[2]
@@ -271,9 +305,83 @@ class Oracle:
         s = 1.0 / np.abs(A).max(axis=2)
         return np.linalg.solve(A * s[:, :, None], (b * s)[:, :, None])[:, :, 0]
 
+    # band storage: ab[b, j, d] = A_b[j, j - kl + d], d = 0 .. kl + ku
+    @staticmethod
+    def _band_pack(A, kl, ku):
+        N = A.shape[0]
+        ab = np.zeros((N, kl + ku + 1), A.dtype)
+        for j in range(N):
+            for d in range(kl + ku + 1):
+                c = j - kl + d
+                if 0 <= c < N:
+                    ab[j, d] = A[j, c]
+        outside = A.copy()
+        for j in range(N):
+            outside[j, max(0, j - kl):min(N, j + ku + 1)] = 0
+        assert not outside.any(), "matrix does not fit the band"
+        return ab
+
+    @staticmethod
+    def _solve_banded(ab, b, kl, ku):
+        """Gaussian elimination WITHOUT pivoting inside the band, row by row, every step
+        vectorised over the batch (BASELINE.json north_star: "dense or banded Gaussian
+        elimination").  ab [B, N, kl+ku+1] real (overwritten), b [B, N] complex (overwritten).
+        The multiplier of (row i, pivot j) is skipped where it is structurally zero (left of the
+        first stored entry of row i in the batch-independent pattern)."""
+        B, N, W = ab.shape
+        first = np.array([j - kl + int(np.argmax(np.any(ab[:, j, :] != 0, axis=0))) for j in range(N)])
+        for j in range(N - 1):
+            piv = ab[:, j, kl]
+            for i in range(j + 1, min(j + kl, N - 1) + 1):
+                if j < first[i]:
+                    continue
+                o = kl - (i - j)
+                l = ab[:, i, o] / piv
+                ab[:, i, o:o + ku + 1] -= l[:, None] * ab[:, j, kl:kl + ku + 1]
+                b[:, i] -= l * b[:, j]
+        for j in range(N - 1, -1, -1):
+            acc = b[:, j]
+            for d in range(1, min(ku, N - 1 - j) + 1):
+                acc = acc - ab[:, j, kl + d] * b[:, j + d]
+            b[:, j] = acc / ab[:, j, kl]
+        return b
+
+    def _helmholtz_banded(self, shift, coef, rhs, im, ik):
+        KL = KU = 8
+        N_r = self.p.N_r
+        if not hasattr(self, "_L0_band"):
+            self._L0_band = self._band_pack(self.L0, KL, KU)
+        q = ((self.n[im] + shift)[:, None] ** 2 / self.r[None, :] ** 2 + self.kappa[ik][:, None] ** 2)
+        ab = np.broadcast_to(-coef * self._L0_band, (len(im), N_r, KL + KU + 1)).copy()
+        ab[:, :, KL] += 1 + coef * q
+        for w in (0, N_r - 1):
+            ab[:, w, :] = 0
+            ab[:, w, KL] = 1
+        return self._solve_banded(ab, np.array(rhs, dtype=self.cplx), KL, KU)
+
+    def _poisson_banded(self, g, im, ik):
+        KL = KU = 12
+        N_r = self.p.N_r
+        if not hasattr(self, "_P_band"):
+            P0 = self.Q.copy()
+            P0[0, :] = self.D1[0]
+            P0[-1, :] = self.D1[-1]
+            self._P_band = self._band_pack(P0, KL, KU)
+        q = self.n[im][:, None] ** 2 / self.r[None, :] ** 2 + self.kappa[ik][:, None] ** 2
+        ab = np.broadcast_to(self._P_band, (len(im), N_r, KL + KU + 1)).copy()
+        ab[:, 1:-1, KL] -= q[:, 1:-1]
+        zero = (np.asarray(im) == 0) & (np.asarray(ik) == self.p.K)
+        ab[zero] = 0
+        ab[zero, :, KL] = 1                                    # O8: mode (0,0) is not projected
+        phi = self._solve_banded(ab, np.array(g, dtype=self.cplx), KL, KU)
+        phi[zero] = 0.0
+        return phi
+
     def _helmholtz(self, shift, coef, rhs, im, ik):
         """(I - coef * (L0 - diag((n+shift)^2/r^2 + kappa^2))) x = rhs for the listed
         modes; rows 0 and N_r-1 replaced by identity (Dirichlet, L2)."""
+        if self.solve == "banded":
+            return self._helmholtz_banded(shift, coef, rhs, im, ik)
         N_r = self.p.N_r
         q = ((self.n[im] + shift)[:, None] ** 2 / self.r[None, :] ** 2
              + self.kappa[ik][:, None] ** 2)                  # [B, N_r]
@@ -289,6 +397,8 @@ class Oracle:
     def _poisson(self, g, im, ik):
         """P phi = g at interior rows, D1 phi = 0 at the wall rows, with
         P = Q - diag(n^2/r^2 + kappa^2), Q = (D1 + 1/r) G~ (L4, R9)."""
+        if self.solve == "banded":
+            return self._poisson_banded(g, im, ik)
         N_r = self.p.N_r
         q = self.n[im][:, None] ** 2 / self.r[None, :] ** 2 + self.kappa[ik][:, None] ** 2
         A = np.broadcast_to(self.Q, (len(im), N_r, N_r)).copy()
@@ -337,7 +447,7 @@ class Oracle:
         if p.heated:
             rhs[3][0, 0, p.K], rhs[3][-1, 0, p.K] = 0.5, -0.5
         nB = len(IM)
-        out = [np.empty((N_r, nB), complex) for _ in range(5)]
+        out = [np.empty((N_r, nB), self.cplx) for _ in range(5)]
         for s in range(0, nB, chunk):
             im, ik = IM[s:s + chunk], IK[s:s + chunk]
             g_ = lambda a: a[:, im, ik].T                    # [B, N_r]
@@ -350,14 +460,17 @@ class Oracle:
             urs = (ups + ums) / 2
             uts = (ups - ums) / 2j
             nn, kk, rr = self.n[im][:, None], self.kappa[ik][:, None], self.r[None, :]
-            g = urs @ self.D1.T + urs / rr + 1j * nn / rr * uts + 1j * kk * uzs
+            g = self._dr_T(urs) + urs / rr + 1j * nn / rr * uts + 1j * kk * uzs
             g[:, 0] = 0.0
             g[:, -1] = 0.0
             # L4 pressure Poisson (all modes except (0,0), O8)
             phi = self._poisson(g, im, ik)
             zero = (im == 0) & (ik == p.K)
             # L5 correct + update
-            urn = urs - phi @ self.Gt.T
+            gphi = self._dr_T(phi)                            # G~ phi: D1 phi with the wall rows zeroed
+            gphi[:, 0] = 0.0
+            gphi[:, -1] = 0.0
+            urn = urs - (gphi if self.solve == "banded" else phi @ self.Gt.T)
             utn = uts - 1j * nn / rr * phi
             uzn = uzs - 1j * kk * phi
             urn[zero] = 0.0                                   # O8: u_r(0,0) := 0
@@ -371,6 +484,15 @@ class Oracle:
             shp = (N_r, p.M + 1, 2 * p.K + 1)
             out = [None if o is None else o.reshape(shp) for o in out]
         return out
+
+    def _dr_T(self, x):
+        """D1 applied along the LAST axis of x [B, N_r] (mode-major arrays of the sub-step)."""
+        if self.solve == "banded":
+            out = np.zeros(x.shape, np.result_type(x.dtype, self.real))
+            for l in range(9):
+                out += self.D1_rows[None, :, l] * x[:, self.s0 + l]
+            return out
+        return x @ self.D1.T
 
     # ---------------------------------------------------------------- O7 step
     def step(self, state, dt):
@@ -446,7 +568,7 @@ class Oracle:
     # ---------------------------------------------------------------- basic states
     def zeros(self):
         p = self.p
-        return np.zeros((p.N_r, p.M + 1, 2 * p.K + 1), complex)
+        return np.zeros((p.N_r, p.M + 1, 2 * p.K + 1), self.cplx)
 
     def base_state_discrete(self):
         """Discrete basic state: u_theta(r), T(r) (and the buoyancy-driven
@@ -462,7 +584,7 @@ class Oracle:
             A[-1, -1] = 1
             b = np.zeros(p.N_r) if rhs is None else rhs.copy()
             b[0], b[-1] = bi, bo
-            return np.linalg.solve(A, b)
+            return np.linalg.solve(A.astype(np.float64), b.astype(np.float64)).astype(self.real)
 
         ur, ut, uz = self.zeros(), self.zeros(), self.zeros()
         ut[:, 0, p.K] = solve(self.L0 - np.diag(1 / r ** 2), p.Re_i, p.Re_o)
@@ -478,4 +600,27 @@ def rel_l2(a_list, b_list):
     """R14 parity norm: ||a - b||_2 / ||b||_2 over the concatenation of all fields."""
     num = sum(np.linalg.norm((a - b).ravel()) ** 2 for a, b in zip(a_list, b_list) if b is not None)
     den = sum(np.linalg.norm(b.ravel()) ** 2 for b in b_list if b is not None)
+    return float(np.sqrt(num / den))
+
+
+def rel_l2_pert(a_list, b_list, K, mean_index=None):
+    """The same norm with the mean mode (0,0) left out of numerator and denominator (SURVEY.md S14:
+    "also report the same norm with mode (0,0) excluded"): the base flow sits in that mode and is
+    10^2..10^4 times larger than the perturbation, so an error confined to the perturbation modes
+    would be discounted by that factor in R14.  Arrays are [N_r, M+1, 2K+1], or [N_r, B] sampled-mode
+    arrays with ``mean_index`` = the positions (along B) of mode (0,0), if any."""
+    num = den = 0.0
+    for a, b in zip(a_list, b_list):
+        if b is None:
+            continue
+        d = np.abs(a - b) ** 2
+        e = np.abs(b) ** 2
+        if b.ndim == 3:
+            d[:, 0, K] = 0.0
+            e[:, 0, K] = 0.0
+        elif mean_index is not None:
+            d[:, mean_index] = 0.0
+            e[:, mean_index] = 0.0
+        num += float(d.sum())
+        den += float(e.sum())
     return float(np.sqrt(num / den))

@@ -10,8 +10,8 @@ def params_of(cfg: dict, **over) -> Params:
     return Params(**d)
 
 
-def oracle_of(cfg: dict, dft="naive", **over) -> Oracle:
-    return Oracle(params_of(cfg, **over), dft=dft)
+def oracle_of(cfg: dict, dft="naive", solve="dense", real=np.float64, **over) -> Oracle:
+    return Oracle(params_of(cfg, **over), dft=dft, solve=solve, real=real)
 
 
 def nf_of(cfg):

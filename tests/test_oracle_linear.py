@@ -107,3 +107,83 @@ def test_modes_subset_equals_full():
     sub = o.substep(st, E, cfg["dt"], modes=(im, ik))
     for a, b in zip(full, sub):
         np.testing.assert_allclose(a[:, im, ik], b, rtol=1e-13, atol=0)
+
+
+# ------------------------------------------------------------------ the thermal diffusivity is 1 / Pr
+def test_temperature_substep_reduces_to_explicit_euler_with_diffusivity_one_over_Pr():
+    """c = 0: T_new = T + dt [ (1/Pr)(T'' + T'/r - (n^2/r^2 + kappa^2) T) + E_T ] at interior nodes, written with
+    ANALYTIC derivatives of a polynomial T (degree 6: the 9-point rows are exact), Pr = 0.7 != 1.  Pins the factor
+    (1 - c)/Pr of L1 (temperature equation; d_t T = ... + (1/Pr) lap T):
+    Pr in place of 1/Pr, or a dropped factor, changes the result by O(dt lap T)."""
+    Pr = 0.7
+    o = Oracle(Params(N_r=24, M=3, K=3, eta=0.5, alpha=2.0, k_theta0=2, Re_i=0.0, Re_o=0.0, Ra=50.0, Pr=Pr, c=0.0))
+    r = o.r
+    x = r - r[0]
+    prof = x * (1 - x) * (1.0 + 0.4 * x - 0.7 * x ** 2 + 0.2 * x ** 3) * (1 + 0.5 * x)       # degree 6, zero at the walls
+    c = np.polynomial.polynomial.polyfromroots([0.0, 1.0]) * -1.0                              # x (1 - x)
+    c = np.polynomial.polynomial.polymul(c, [1.0, 0.4, -0.7, 0.2])
+    c = np.polynomial.polynomial.polymul(c, [1.0, 0.5])
+    np.testing.assert_allclose(np.polynomial.polynomial.polyval(x, c), prof, atol=1e-14)
+    d1 = np.polynomial.polynomial.polyval(x, np.polynomial.polynomial.polyder(c))
+    d2 = np.polynomial.polynomial.polyval(x, np.polynomial.polynomial.polyder(c, 2))
+    st = [o.zeros() for _ in range(5)]
+    amp = {(1, 4): 1.0 + 0.5j, (2, 1): -0.3 + 2.0j, (0, 5): 0.7 - 0.2j}
+    for (m, kk), a in amp.items():
+        st[3][:, m, kk] = a * prof
+    rng = np.random.default_rng(5)
+    E = [o.zeros(), o.zeros(), o.zeros(), rng.standard_normal(st[0].shape) + 1j * rng.standard_normal(st[0].shape)]
+    dt = 1e-3
+    out = o.substep(st, E, dt)
+    for (m, kk), a in amp.items():
+        q = o.n[m] ** 2 / r ** 2 + o.kappa[kk] ** 2
+        want = a * prof + dt * ((1.0 / Pr) * a * (d2 + d1 / r - q * prof) + E[3][:, m, kk])
+        got = out[3][:, m, kk]
+        scale = np.abs(dt * a * (d2 + d1 / r - q * prof)).max()
+        assert scale > 1e-3                                   # the diffusion term is what is being tested
+        np.testing.assert_allclose(got[1:-1], want[1:-1], rtol=0, atol=1e-10 * scale)
+        wrong = a * prof + dt * (Pr * a * (d2 + d1 / r - q * prof) + E[3][:, m, kk])
+        assert np.abs(got[1:-1] - wrong[1:-1]).max() > 0.1 * scale
+
+
+def _cheb_dd(N):
+    x = np.cos(np.pi * np.arange(N + 1) / N)
+    cc = np.ones(N + 1)
+    cc[0] = cc[-1] = 2
+    cc *= (-1) ** np.arange(N + 1)
+    X = np.tile(x, (N + 1, 1)).T
+    D = np.outer(cc, 1 / cc) / (X - X.T + np.eye(N + 1))
+    D -= np.diag(D.sum(1))
+    return D, x
+
+
+@pytest.mark.parametrize("Pr", [0.7, 3.0])
+def test_conduction_mode_decays_at_the_diffusion_eigenvalue_over_Pr(Pr):
+    """A temperature perturbation in one axial mode with the fluid at rest obeys d_t T = (1/Pr)(DD* - kappa^2) T,
+    T = 0 at the walls, so after the transients it decays at lambda_1 / Pr with lambda_1 the leading
+    eigenvalue of DD* - kappa^2 = d^2/dr^2 + (1/r) d/dr - kappa^2, computed here by Chebyshev collocation (a
+    discretisation independent of the oracle's).  The implicit sub-step with no explicit term is the
+    Crank-Nicolson integrator of that equation: pins both (1 - c)/Pr in L1 and c dt/Pr in L2."""
+    eta, kap = 0.5, 3.0
+    D, xc = _cheb_dd(40)
+    rc = eta / (1 - eta) + 0.5 * (1 - xc)
+    D = D / (-0.5)
+    A = D @ D + np.diag(1 / rc) @ D - kap ** 2 * np.eye(41)
+    lam = np.sort(np.linalg.eigvals(A[1:-1, 1:-1]).real)[::-1]
+    assert lam[0] == pytest.approx(-(np.pi ** 2 + kap ** 2), rel=2e-2)     # close to the planar value
+    o = Oracle(Params(N_r=32, M=1, K=1, eta=eta, alpha=kap, k_theta0=1, Re_i=0.0, Re_o=0.0, Ra=1.0, Pr=Pr))
+    st = [o.zeros() for _ in range(5)]
+    x = o.r - o.r[0]
+    st[3][:, 0, 2] = x * (1 - x) * (1 + x)
+    st[3][:, 0, 0] = np.conj(st[3][:, 0, 2])
+    E = [o.zeros() for _ in range(4)]
+    dt = 2e-3 * Pr
+    t0, t1 = 0.3 * Pr, 0.4 * Pr
+    n0, n1 = round(t0 / dt), round(t1 / dt)
+    amp = {}
+    for i in range(1, n1 + 1):
+        st = o.substep(st, E, dt)
+        if i in (n0, n1):
+            amp[i] = np.linalg.norm(st[3][:, 0, 2])
+    rate = np.log(amp[n1] / amp[n0]) / ((n1 - n0) * dt)
+    assert rate == pytest.approx(lam[0] / Pr, rel=1e-3)
+    assert abs(rate - lam[0] * Pr) > 0.3 * abs(rate)          # Pr in place of 1 / Pr would be far off

@@ -146,3 +146,33 @@ def test_nodes_subset_equals_full():
     sub = o.nonlinear(*fs, nodes=[0, 6, 13])
     for a, b in zip(full, sub):
         np.testing.assert_array_equal(a[[0, 6, 13]], b)
+
+
+# ------------------------------------------------------------------ T9 spatial order
+def test_T9_spatial_order_of_the_nonlinear_term_on_the_uniform_grid():
+    """Pin T9: for a non-polynomial field the error of N falls at >= 7th order under N_r doubling on
+    the uniform grid (nine-point rows: degree-8 exactness).  Field: azimuthal flow V(r) = J_1(2.3 r)
+    (a Bessel function) in mode (0,0) and a radial velocity a(r) e^{i(n theta + kappa z)} + c.c. with
+    a = e^{-r}: the (m1,k1) coefficient of N_theta is then exactly -a (V' + V / r) (u_r d_r u_theta + u_r u_theta / r;
+    every other product lands in other modes), and d_r V is the only place the finite differences enter."""
+    from scipy.special import jv, jvp
+    errs = []
+    sizes = (12, 24, 48)
+    for N_r in sizes:
+        o = Oracle(Params(N_r=N_r, M=4, K=4, eta=0.5, alpha=1.5, k_theta0=2, Re_i=0.0, Re_o=0.0, grid=0))
+        r = o.r
+        ur, ut, uz = o.zeros(), o.zeros(), o.zeros()
+        V, dV = jv(1, 2.3 * r), 2.3 * jvp(1, 2.3 * r)
+        a = np.exp(-r) * (0.8 - 0.3j)
+        ut[:, 0, 4] = V
+        ur[:, 1, 5] = a
+        N = o.nonlinear(ur, ut, uz)
+        exact = -a * (dV + V / r)
+        errs.append(np.abs(N[1][:, 1, 5] - exact).max() / np.abs(exact).max())
+        # and N_r of the same pair: (u_theta / r) d_theta u_r = (V / r) i n a, no radial derivative: exact at any N_r
+        exact_r = -(V / r) * 1j * o.n[1] * a
+        assert np.abs(N[0][:, 1, 5] - exact_r).max() <= 1e-13 * np.abs(exact_r).max()
+    assert errs[0] > 1e-9                                      # resolvable truncation error on the coarse grid
+    orders = [np.log(errs[i] / errs[i + 1]) / np.log((sizes[i + 1] - 1) / (sizes[i] - 1)) for i in range(2)]
+    assert orders[0] >= 7.0, (errs, orders)
+    assert orders[1] >= 7.0 or errs[2] <= 1e-13, (errs, orders)

@@ -82,3 +82,18 @@ def test_m0_row_takes_real_part():
     g = f.copy()
     g[:, 0, :] = 0.5 * (f[:, 0, :] + np.conj(f[:, 0, ::-1]))
     np.testing.assert_allclose(o.to_physical(f), o.to_physical(g), atol=1e-14)
+
+
+@pytest.mark.parametrize("M,K", [(256, 8), (8, 256), (512, 4), (4, 512), (128, 128)])
+def test_library_fft_pinned_to_naive_sums_at_the_long_lengths(M, K):
+    """The ``dft="fft"`` backend (numpy FFT as a library primitive) against the naive sums at the line lengths of
+    BASELINE.json configs[2..4] (384, 768, 1536), where the 20-step parity runs use it as the checker."""
+    p = Params(N_r=9, M=M, K=K, eta=0.5, alpha=3.0, k_theta0=1, Re_i=1.0, Re_o=0.0)
+    o, of = Oracle(p), Oracle(p, dft="fft")
+    rng = np.random.default_rng(11)
+    f = (rng.standard_normal((2, M + 1, 2 * K + 1)) + 1j * rng.standard_normal((2, M + 1, 2 * K + 1)))
+    u, uf = o.to_physical(f), of.to_physical(f)
+    assert np.abs(u - uf).max() <= 1e-13 * np.abs(u).max()
+    x = rng.standard_normal(u.shape)
+    a, b = o.from_physical(x), of.from_physical(x)
+    assert np.abs(a - b).max() <= 1e-13 * np.abs(a).max()
