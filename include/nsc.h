@@ -171,6 +171,17 @@ int nsc_set_profiling(nsc_ctx* ctx, int on);
 int nsc_profile_read(nsc_ctx* ctx, double* h_ms, long long* h_count);
 const char* nsc_kernel_name(int id);
 
+
+/* Number of times nsc_step replayed its captured CUDA graph on this context (0 on the legacy default
+ * stream or with profiling on, where the kernels are launched one by one).  For tests and reports. */
+long long nsc_graph_replays(const nsc_ctx* ctx);
+
+/* Measured fp64 peak of a device: a register-only
+ * kernel on every SM, timed with CUDA events, best of six runs.  kind 0: DFMA only (2 flop each);
+ * kind 1: DADD and DMUL alternating (1 flop each).  device: CUDA ordinal, -1 = current.
+ * *h_tflops (HOST double) receives TFLOP/s.  Synchronises the device; needs no context. */
+int nsc_fp64_peak(int kind, int device, double* h_tflops);
+
 #ifdef __cplusplus
 }
 #endif

@@ -333,11 +333,13 @@ int nsc_step(nsc_ctx* c, double dt) {
     // replayed: small configurations are launch-bound.  With per-kernel profiling on (event brackets), or if
     // capture is not possible, the kernels are launched one by one.
     if (c->use_graph && !c->profiling) {
+        // set-up kernels stay outside the graph; a no-op unless dt changed since the factors were built (another
+        // call, e.g. nsc_substep with its own dt, may have rebuilt them in place since the graph was captured)
+        int rc = ensure_factors(c, dt);
+        if (rc) return rc;
         const bool stale = !c->graph_exec || c->graph_dt != dt || c->graph_stream != c->stream || c->graph_gen != c->ptr_gen;
         if (stale) {
             drop_graph(c);
-            int rc = ensure_factors(c, dt);             // set-up kernels stay outside the graph
-            if (rc) return rc;
             cudaGraph_t g = nullptr;
             const long long l0 = c->launches;
             if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
@@ -350,19 +352,19 @@ int nsc_step(nsc_ctx* c, double dt) {
                     c->graph_launches = c->launches - l0;
                 } else {
                     c->graph_exec = nullptr;
-                    c->use_graph = false;                // fall back to plain launches for good
+                    c->use_graph = false;                // capture works on this stream but the graph does not: plain launches for good
                 }
                 if (g) cudaGraphDestroy(g);
                 cudaGetLastError();
             } else {
-                cudaGetLastError();
-                c->use_graph = false;
+                cudaGetLastError();                      // no capture on this stream (legacy default stream): plain launches for this call only
             }
             c->launches = l0;
         }
         if (c->graph_exec) {
             NSC_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
             c->launches += c->graph_launches;
+            c->graph_replays += 1;
             return NSC_OK;
         }
     }
@@ -474,5 +476,7 @@ const char* nsc_last_error(const nsc_ctx* c) { return c ? c->err.c_str() : g_cre
 long long nsc_device_bytes(const nsc_ctx* c) { return c ? c->dev_bytes : 0; }
 
 long long nsc_launch_count(const nsc_ctx* c) { return c ? c->launches : 0; }
+
+long long nsc_graph_replays(const nsc_ctx* c) { return c ? c->graph_replays : 0; }
 
 }  // extern "C"

@@ -88,7 +88,7 @@ struct nsc_ctx {
     cudaGraphExec_t graph_exec = nullptr;
     double graph_dt = 0.0;
     cudaStream_t graph_stream = nullptr;
-    long long graph_gen = -1, ptr_gen = 0, graph_launches = 0;
+    long long graph_gen = -1, ptr_gen = 0, graph_launches = 0, graph_replays = 0;
     int n_slices = 2;                                 // mode slices of the linear stage (NSC_LIN_SLICES overrides)
     cudaStream_t slice_stream[NSC_MAX_SLICES] = {};   // their streams
     cudaEvent_t slice_ev[NSC_MAX_SLICES + 1] = {};    // [0] fork, [1 + s] join of slice s

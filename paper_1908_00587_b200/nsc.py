@@ -21,7 +21,8 @@ EXPORTS = (
     "nsc_create", "nsc_create_ex", "nsc_destroy", "nsc_set_stream", "nsc_get_grid",
     "nsc_set_state", "nsc_get_state", "nsc_set_state_host", "nsc_get_state_host",
     "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_step_iterated", "nsc_nusselt", "nsc_probe", "nsc_last_error", "nsc_device_bytes",
-    "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name",
+    "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name", "nsc_graph_replays",
+    "nsc_fp64_peak",
 )
 NSC_NKERN = 11
 
@@ -82,8 +83,12 @@ def load_library() -> C.CDLL:
     lib.nsc_profile_read.argtypes = [vp, C.POINTER(dbl), C.POINTER(C.c_longlong)]
     lib.nsc_kernel_name.argtypes = [i32]
     lib.nsc_kernel_name.restype = C.c_char_p
+    lib.nsc_graph_replays.argtypes = [vp]
+    lib.nsc_graph_replays.restype = C.c_longlong
+    lib.nsc_fp64_peak.argtypes = [i32, i32, C.POINTER(dbl)]
     for name in EXPORTS:
-        if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count", "nsc_kernel_name"):
+        if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count", "nsc_kernel_name",
+                        "nsc_graph_replays"):
             getattr(lib, name).restype = i32
     _lib = lib
     return lib
@@ -101,6 +106,16 @@ def _ptr(t):
     if t.dtype != torch.complex128 or not t.is_contiguous():
         raise ValueError("device buffers must be contiguous complex128")
     return C.c_void_p(t.data_ptr())
+
+
+def fp64_peak(kind: int = 0, device: int = -1) -> float:
+    """nsc_fp64_peak: measured fp64 TFLOP/s of the device (kind 0 DFMA, kind 1 DADD + DMUL)."""
+    lib = load_library()
+    v = C.c_double(0.0)
+    rc = lib.nsc_fp64_peak(kind, device, C.byref(v))
+    if rc != NSC_OK:
+        raise NscError(rc, "nsc_fp64_peak failed (no CUDA device?)")
+    return v.value
 
 
 class Context:
@@ -210,6 +225,9 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self._lib.nsc_launch_count(self._h))
+
+    def graph_replays(self) -> int:
+        return int(self._lib.nsc_graph_replays(self._h))
 
     def set_profiling(self, on: bool):
         self._check(self._lib.nsc_set_profiling(self._h, int(bool(on))))

@@ -20,7 +20,7 @@ def test_header_symbols_are_exported(lib):
     from paper_1908_00587_b200 import nsc
     hdr = open(os.path.join(ROOT, "include", "nsc.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(nsc_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(nsc_[a-z0-9_]+)\s*\(", hdr))
     assert declared, "no declarations found in include/nsc.h"
     for name in declared:
         assert hasattr(lib, name), f"{name} declared in nsc.h but not exported by libnsc.so"
