@@ -30,6 +30,8 @@ tests/test_oracle_transforms.py) so that the large configurations finish.
 
 Linear solves are dense Gaussian elimination with partial pivoting after row
 equilibration (LAPACK ``gesv`` through ``numpy.linalg.solve`` on row-scaled matrices).
+``solve="c"`` is the same banded elimination written in plain C (oracle/nsc_oracle_sub.c, the whole
+sub-step L1-L5 per mode, OpenMP over modes), pinned to both numpy backends.
 ``solve="banded"`` is the second backend BASELINE.json north_star allows ("dense or banded
 Gaussian elimination"): the same matrices held by diagonals and eliminated row by row without
 pivoting, vectorised over the Fourier modes, and the radial operators applied through their
@@ -37,15 +39,20 @@ pivoting, vectorised over the Fourier modes, and the radial operators applied th
 (tests/test_oracle_banded.py) and exists so that 20-step runs at the large configurations
 finish; plain numpy throughout, so it also runs in ``real=numpy.longdouble`` (SURVEY.md 8(c):
 "oracle(double) vs oracle(long double) after 20 steps is reported as the floor"), where the
-tables are kept in extended precision instead of being rounded to double.
+tables are kept in extended precision instead of being rounded to double.  The sub-step treats
+chunks of Fourier modes independently; with the banded backend the chunks are
+handed to a thread pool (outer-loop parallelism only, as SURVEY.md section 7 plans for the oracle).
 
 Parity unpinned (defined by the algorithm only): the pressure field,
 the O(dt^2) tangential wall slip, and the aliased extreme modes |k| = K, m = M.
 """
 from __future__ import annotations
 
+import concurrent.futures
 import dataclasses
+import os
 import numpy as np
+import scipy.fft as _fft          # pocketfft, the routines behind numpy.fft, with a ``workers`` argument
 
 LD = np.longdouble
 
@@ -164,13 +171,14 @@ class Oracle:
     """One Taylor-Couette configuration; methods follow O3..O8 in SURVEY.md 8(c)."""
 
     def __init__(self, p: Params, dft: str = "naive", solve: str = "dense", real=np.float64):
-        if solve not in ("dense", "banded"):
-            raise ValueError("solve must be 'dense' or 'banded'")
+        if solve not in ("dense", "banded", "c"):
+            raise ValueError("solve must be 'dense', 'banded' or 'c'")
         if real is not np.float64 and solve != "banded":
-            raise ValueError("extended precision needs solve='banded' (LAPACK is double only)")
+            raise ValueError("extended precision needs solve='banded' (LAPACK and the C backend are double only)")
         self.p = p
         self.dft = dft
         self.solve = solve
+        self.band_ops = solve != "dense"                     # radial operators through their 9-point rows
         self.real = real
         self.cplx = np.result_type(real, np.complex64)       # complex128 / clongdouble
         N_r = p.N_r
@@ -216,8 +224,8 @@ class Oracle:
             pad = np.zeros(fh.shape[:-2] + (p.n_theta // 2 + 1, p.n_z), self.cplx)
             kk = np.arange(-p.K, p.K + 1) % p.n_z
             pad[..., :p.M + 1, kk] = fh
-            half = np.fft.ifft(pad, axis=-1) * p.n_z
-            return np.fft.irfft(half, n=p.n_theta, axis=-2) * p.n_theta
+            half = _fft.ifft(pad, axis=-1, workers=-1) * p.n_z
+            return _fft.irfft(half, n=p.n_theta, axis=-2, workers=-1) * p.n_theta
         half = fh @ self.Ez                                   # sum over k -> [..., M+1, N_z]
         half = half * self.cm[:, None]
         return np.real(np.swapaxes(np.swapaxes(half, -1, -2) @ self.Et, -1, -2))
@@ -228,7 +236,7 @@ class Oracle:
         u: real [..., N_theta, N_z] -> [..., M+1, 2K+1]."""
         p = self.p
         if self.dft == "fft":
-            h = np.fft.fft(np.fft.rfft(u, axis=-2), axis=-1) / (p.n_theta * p.n_z)
+            h = _fft.fft(_fft.rfft(u, axis=-2, workers=-1), axis=-1, workers=-1) / (p.n_theta * p.n_z)
             kk = np.arange(-p.K, p.K + 1) % p.n_z
             return h[..., :p.M + 1, :][..., kk]
         t = np.conj(self.Et) @ u                              # sum over a -> [..., M+1, N_z]
@@ -245,7 +253,7 @@ class Oracle:
 
     def d_r(self, f):
         """Radial derivative: sum_{l in S(j)} D1[j,l] f_l (N1)."""
-        if self.solve == "banded":
+        if self.band_ops:
             return self._rows9(self.D1_rows, f)
         return np.einsum("jl,lmk->jmk", self.D1, f)
 
@@ -254,7 +262,7 @@ class Oracle:
         shift = +-1: L_+- acting on u_+- = u_r +- i u_theta (O5)."""
         q = ((self.n[None, :, None] + shift) ** 2 / self.r[:, None, None] ** 2
              + self.kappa[None, None, :] ** 2)
-        if self.solve == "banded":
+        if self.band_ops:
             return self._rows9(self.L0_rows, f) - q * f
         return np.einsum("jl,lmk->jmk", self.L0, f) - q * f
 
@@ -265,7 +273,7 @@ class Oracle:
                 + 1j * self.kappa[None, None, :] * uz)
 
     # ---------------------------------------------------------------- O4 nonlinear term
-    def nonlinear(self, ur, ut, uz, T=None, nodes=None):
+    def nonlinear(self, ur, ut, uz, T=None, nodes=None, workers=1):
         """N = -(u.grad)u with the cylindrical curvature terms, + (Ra/Pr) T^ e_z, and
         N_T = -(u.grad)T (N1..N6; convective form, R7).  Evaluated at every radial node
         (walls included) or at the listed ``nodes`` only (same values; used for sampled
@@ -273,6 +281,12 @@ class Oracle:
         p = self.p
         fields = [ur, ut, uz] + ([T] if p.heated else [])
         js = np.arange(p.N_r) if nodes is None else np.asarray(nodes)
+        if workers > 1 and len(js) > 16:
+            # radial nodes are independent: chunks of 16 nodes on a thread pool, same values
+            parts = [js[i:i + 16] for i in range(0, len(js), 16)]
+            with concurrent.futures.ThreadPoolExecutor(max_workers=workers) as ex:
+                res = list(ex.map(lambda q: self.nonlinear(ur, ut, uz, T, nodes=q), parts))
+            return [np.concatenate([r_[i] for r_ in res]) for i in range(len(fields))]
         i_n = 1j * self.n[None, :, None]
         i_k = 1j * self.kappa[None, None, :]
         rj = self.r[js][:, None, None]
@@ -280,7 +294,7 @@ class Oracle:
         for f in fields:
             fj = f[js]
             ph.append(self.to_physical(fj))
-            d_r.append(self.to_physical(self._rows9(self.D1_rows, f, js) if self.solve == "banded"
+            d_r.append(self.to_physical(self._rows9(self.D1_rows, f, js) if self.band_ops
                                         else np.einsum("jl,lmk->jmk", self.D1[js], f)))
             d_t.append(self.to_physical(i_n * fj))
             d_z.append(self.to_physical(i_k * fj))
@@ -325,25 +339,26 @@ class Oracle:
     def _solve_banded(ab, b, kl, ku):
         """Gaussian elimination WITHOUT pivoting inside the band, row by row, every step
         vectorised over the batch (BASELINE.json north_star: "dense or banded Gaussian
-        elimination").  ab [B, N, kl+ku+1] real (overwritten), b [B, N] complex (overwritten).
-        The multiplier of (row i, pivot j) is skipped where it is structurally zero (left of the
-        first stored entry of row i in the batch-independent pattern)."""
-        B, N, W = ab.shape
-        first = np.array([j - kl + int(np.argmax(np.any(ab[:, j, :] != 0, axis=0))) for j in range(N)])
+        elimination").  ab [N, kl+ku+1, B] real (overwritten; batch index last so that every
+        vector operation is contiguous), b [N, B] complex (overwritten).  The multiplier of
+        (row i, pivot j) is skipped where it is structurally zero: left of the first stored entry
+        of row i in the batch-independent pattern."""
+        N, W, B = ab.shape
+        first = np.array([j - kl + int(np.argmax(np.any(ab[j] != 0, axis=1))) for j in range(N)])
         for j in range(N - 1):
-            piv = ab[:, j, kl]
+            piv = ab[j, kl]
             for i in range(j + 1, min(j + kl, N - 1) + 1):
                 if j < first[i]:
                     continue
                 o = kl - (i - j)
-                l = ab[:, i, o] / piv
-                ab[:, i, o:o + ku + 1] -= l[:, None] * ab[:, j, kl:kl + ku + 1]
-                b[:, i] -= l * b[:, j]
+                l = ab[i, o] / piv
+                ab[i, o:o + ku + 1] -= l[None, :] * ab[j, kl:kl + ku + 1]
+                b[i] -= l * b[j]
         for j in range(N - 1, -1, -1):
-            acc = b[:, j]
+            acc = b[j]
             for d in range(1, min(ku, N - 1 - j) + 1):
-                acc = acc - ab[:, j, kl + d] * b[:, j + d]
-            b[:, j] = acc / ab[:, j, kl]
+                acc = acc - ab[j, kl + d] * b[j + d]
+            b[j] = acc / ab[j, kl]
         return b
 
     def _helmholtz_banded(self, shift, coef, rhs, im, ik):
@@ -351,13 +366,13 @@ class Oracle:
         N_r = self.p.N_r
         if not hasattr(self, "_L0_band"):
             self._L0_band = self._band_pack(self.L0, KL, KU)
-        q = ((self.n[im] + shift)[:, None] ** 2 / self.r[None, :] ** 2 + self.kappa[ik][:, None] ** 2)
-        ab = np.broadcast_to(-coef * self._L0_band, (len(im), N_r, KL + KU + 1)).copy()
-        ab[:, :, KL] += 1 + coef * q
+        q = ((self.n[im] + shift)[None, :] ** 2 / self.r[:, None] ** 2 + self.kappa[ik][None, :] ** 2)   # [N_r, B]
+        ab = np.broadcast_to((-coef * self._L0_band)[:, :, None], (N_r, KL + KU + 1, len(im))).copy()
+        ab[:, KL, :] += 1 + coef * q
         for w in (0, N_r - 1):
-            ab[:, w, :] = 0
-            ab[:, w, KL] = 1
-        return self._solve_banded(ab, np.array(rhs, dtype=self.cplx), KL, KU)
+            ab[w] = 0
+            ab[w, KL] = 1
+        return self._solve_banded(ab, np.array(rhs.T, dtype=self.cplx), KL, KU).T
 
     def _poisson_banded(self, g, im, ik):
         KL = KU = 12
@@ -367,13 +382,13 @@ class Oracle:
             P0[0, :] = self.D1[0]
             P0[-1, :] = self.D1[-1]
             self._P_band = self._band_pack(P0, KL, KU)
-        q = self.n[im][:, None] ** 2 / self.r[None, :] ** 2 + self.kappa[ik][:, None] ** 2
-        ab = np.broadcast_to(self._P_band, (len(im), N_r, KL + KU + 1)).copy()
-        ab[:, 1:-1, KL] -= q[:, 1:-1]
+        q = self.n[im][None, :] ** 2 / self.r[:, None] ** 2 + self.kappa[ik][None, :] ** 2
+        ab = np.broadcast_to(self._P_band[:, :, None], (N_r, KL + KU + 1, len(im))).copy()
+        ab[1:-1, KL, :] -= q[1:-1]
         zero = (np.asarray(im) == 0) & (np.asarray(ik) == self.p.K)
-        ab[zero] = 0
-        ab[zero, :, KL] = 1                                    # O8: mode (0,0) is not projected
-        phi = self._solve_banded(ab, np.array(g, dtype=self.cplx), KL, KU)
+        ab[:, :, zero] = 0
+        ab[:, KL, zero] = 1                                    # O8: mode (0,0) is not projected
+        phi = self._solve_banded(ab, np.array(g.T, dtype=self.cplx), KL, KU).T
         phi[zero] = 0.0
         return phi
 
@@ -412,7 +427,7 @@ class Oracle:
         phi[zero] = 0.0
         return phi
 
-    def substep(self, state, E, dt, modes=None, chunk=2048):
+    def substep(self, state, E, dt, modes=None, chunk=None):
         """One implicit sub-step L1..L5 from ``state`` = (ur, ut, uz, T, p) with explicit
         term E = [E_r, E_theta, E_z, (E_T)].  ``modes``: optional (im, ik) index arrays to
         restrict to sampled modes (returns arrays [N_r, B]); default all modes."""
@@ -420,6 +435,8 @@ class Oracle:
         c = p.c
         ur, ut, uz, T, pr = state
         N_r = p.N_r
+        if chunk is None:
+            chunk = 2048 if self.solve == "dense" else 4096
         full = modes is None
         if full:
             IM, IK = np.meshgrid(np.arange(p.M + 1), np.arange(2 * p.K + 1), indexing="ij")
@@ -448,7 +465,16 @@ class Oracle:
             rhs[3][0, 0, p.K], rhs[3][-1, 0, p.K] = 0.5, -0.5
         nB = len(IM)
         out = [np.empty((N_r, nB), self.cplx) for _ in range(5)]
-        for s in range(0, nB, chunk):
+        if self.solve == "c":
+            self._substep_c(state, E, dt, IM, IK, out)
+            if not p.heated:
+                out[3] = None
+            if full:
+                shp = (N_r, p.M + 1, 2 * p.K + 1)
+                out = [None if o is None else o.reshape(shp) for o in out]
+            return out
+
+        def solve_chunk(s):
             im, ik = IM[s:s + chunk], IK[s:s + chunk]
             g_ = lambda a: a[:, im, ik].T                    # [B, N_r]
             # L2 Helmholtz solves
@@ -478,6 +504,14 @@ class Oracle:
             for o, v in zip(out, (urn, utn, uzn, Tn, pn)):
                 if v is not None:
                     o[:, s:s + chunk] = v.T
+
+        starts = list(range(0, nB, chunk))
+        if self.solve == "banded" and len(starts) > 1:
+            with concurrent.futures.ThreadPoolExecutor(max_workers=min(len(starts), os.cpu_count() or 1)) as ex:
+                list(ex.map(solve_chunk, starts))
+        else:
+            for s in starts:
+                solve_chunk(s)
         if not p.heated:
             out[3] = None
         if full:
@@ -485,25 +519,62 @@ class Oracle:
             out = [None if o is None else o.reshape(shp) for o in out]
         return out
 
+    def _substep_c(self, state, E, dt, IM, IK, out):
+        """The same sub-step for the listed modes by oracle/nsc_oracle_sub.c (plain C, OpenMP over modes)."""
+        import ctypes as C
+        p = self.p
+        if not hasattr(self, "_clib"):
+            from oracle import build_c
+            self._clib = C.CDLL(build_c.build())
+            self._clib.orc_substep.restype = C.c_int
+            P0 = self.Q.copy()
+            P0[0, :] = self.D1[0]
+            P0[-1, :] = self.D1[-1]
+            self._P_band_c = np.ascontiguousarray(self._band_pack(P0, 12, 12))
+        ptr = lambda a: C.c_void_p(0) if a is None else a.ctypes.data_as(C.c_void_p)
+        keep = []
+
+        def arr(a, dt_):
+            if a is None:
+                return None
+            b = np.ascontiguousarray(a, dtype=dt_)
+            keep.append(b)
+            return b
+
+        fields = [arr(a, np.complex128) for a in state]
+        Es = [arr(a, np.complex128) for a in E] + [None] * (4 - len(E))
+        tabs = [arr(a, np.float64) for a in (self.r, self.n, self.kappa, self.D1_rows, self.L0_rows)]
+        s0 = arr(self.s0, np.int32)
+        im, ik = arr(IM, np.int32), arr(IK, np.int32)
+        rc = self._clib.orc_substep(
+            C.c_int(p.N_r), C.c_int(p.M + 1), C.c_int(2 * p.K + 1), C.c_int(p.K), C.c_int(4 if p.heated else 3),
+            ptr(tabs[0]), ptr(tabs[1]), ptr(tabs[2]), ptr(tabs[3]), ptr(tabs[4]), ptr(s0), ptr(self._P_band_c),
+            *[ptr(a) for a in fields], *[ptr(a) for a in Es],
+            C.c_double(dt), C.c_double(p.c), C.c_double(p.Pr), C.c_double(p.Re_i), C.c_double(p.Re_o),
+            ptr(im), ptr(ik), C.c_int(len(im)), *[ptr(o) for o in out])
+        if rc != 0:
+            raise MemoryError("orc_substep failed")
+
     def _dr_T(self, x):
         """D1 applied along the LAST axis of x [B, N_r] (mode-major arrays of the sub-step)."""
         if self.solve == "banded":
-            out = np.zeros(x.shape, np.result_type(x.dtype, self.real))
+            xt = np.ascontiguousarray(x.T)                    # [N_r, B]
+            out = np.zeros(xt.shape, np.result_type(x.dtype, self.real))
             for l in range(9):
-                out += self.D1_rows[None, :, l] * x[:, self.s0 + l]
-            return out
+                out += self.D1_rows[:, l][:, None] * xt[self.s0 + l]
+            return np.ascontiguousarray(out.T)
         return x @ self.D1.T
 
     # ---------------------------------------------------------------- O7 step
-    def step(self, state, dt):
+    def step(self, state, dt, workers=1):
         """Predictor-corrector step (R10: c = 1/2, one corrector pass).
         N0 = N(u^n); u^1 = substep(N0) (its pressure discarded); N1 = N(u^1);
         u^{n+1} = substep(c N1 + (1-c) N0), both sub-steps starting from (u^n, T^n, p^n)."""
         c = self.p.c
         nf = 4 if self.p.heated else 3
-        N0 = self.nonlinear(*state[:nf])
+        N0 = self.nonlinear(*state[:nf], workers=workers)
         s1 = self.substep(state, N0, dt)
-        N1 = self.nonlinear(*s1[:nf])
+        N1 = self.nonlinear(*s1[:nf], workers=workers)
         return self.substep(state, [c * a + (1 - c) * b for a, b in zip(N1, N0)], dt)
 
     # ---------------------------------------------------------------- NEXT-1: iterated corrector

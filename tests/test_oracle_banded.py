@@ -23,6 +23,7 @@ def test_band_storage_matches_the_dense_matrix():
     x = rng.standard_normal(21)
     for A, kl, ku in ((o.L0, 8, 8), (o.Q, 12, 12), (o.D1, 8, 8)):
         ab = Oracle._band_pack(A, kl, ku)
+        assert ab.shape == (21, kl + ku + 1)
         y = np.zeros(21)
         for j in range(21):
             for d in range(kl + ku + 1):
@@ -76,6 +77,31 @@ def test_banded_operators_and_substep_equal_dense(ci, N_r, M, K):
     assert rel_l2_pert(sb[:nf], sd[:nf], K) <= 1e-11
 
 
+@pytest.mark.parametrize("ci,N_r,M,K,grid,c", [(0, 32, 8, 8, 1, 0.5), (2, 24, 4, 6, 1, 0.5), (2, 17, 3, 5, 0, 0.7), (1, 9, 2, 2, 1, 1.0)])
+def test_c_backend_substep_equals_dense_and_banded(ci, N_r, M, K, grid, c):
+    """solve="c" (oracle/nsc_oracle_sub.c: the whole sub-step L1-L5 per mode in plain C) against the dense and
+    the numpy banded backends: full mode set and a sampled subset, heated and unheated, both grids, c != 1/2."""
+    cfg = dict(synth.scaled_config(ci, N_r=N_r, M=M, K=K), grid=grid)
+    nf = nf_of(cfg)
+    od, ob, oc = oracle_of(cfg, c=c), oracle_of(cfg, solve="banded", c=c), oracle_of(cfg, solve="c", c=c)
+    st = synth.make_state(cfg, od.r)
+    rng = np.random.default_rng(3)
+    st[4] = 3.0 * (rng.standard_normal(st[0].shape) + 1j * rng.standard_normal(st[0].shape))
+    U = max(abs(cfg["Re_i"]), abs(cfg["Re_o"]))
+    E = [0.1 * U * U * (rng.standard_normal(st[0].shape) + 1j * rng.standard_normal(st[0].shape)) for _ in range(nf)]
+    sd, sb, sc = (o.substep(st, E, cfg["dt"]) for o in (od, ob, oc))
+    assert sc[3] is None if nf == 3 else sc[3] is not None
+    assert rel_l2(sc[:nf], sd[:nf]) <= 1e-12 and rel_l2(sc[:nf], sb[:nf]) <= 1e-12
+    assert rel_l2_pert(sc[:nf], sd[:nf], K) <= 1e-11
+    assert rel_l2([sc[4]], [sd[4]]) <= 1e-7                   # pressure: parity unpinned (phi / dt)
+    np.testing.assert_array_equal(sc[0][:, 0, K], 0.0)        # O8: u_r(0,0) := 0
+    im, ik = np.array([0, 0, M, 1]), np.array([K, K + 1, 0, 2 * K])
+    sub = oc.substep(st, E, cfg["dt"], modes=(im, ik))
+    for a, b in zip(sc, sub):
+        if a is not None:
+            np.testing.assert_array_equal(a[:, im, ik], b)
+
+
 @pytest.mark.parametrize("ci,nsteps", [(0, 20), (1, 6)])
 def test_banded_backend_steps_at_full_cfg1_cfg2(ci, nsteps):
     """The banded backend pinned to the dense one to <= 1e-12 (R14 norm) on BASELINE.json configs[0] (the 20
@@ -83,15 +109,17 @@ def test_banded_backend_steps_at_full_cfg1_cfg2(ci, nsteps):
     both at full size."""
     cfg = synth.config(ci)
     nf = nf_of(cfg)
-    od, ob = oracle_of(cfg, dft="fft"), oracle_of(cfg, dft="fft", solve="banded")
-    a = b = synth.make_state(cfg, od.r)
+    od, ob, oc = oracle_of(cfg, dft="fft"), oracle_of(cfg, dft="fft", solve="banded"), oracle_of(cfg, dft="fft", solve="c")
+    a = b = c = synth.make_state(cfg, od.r)
     for _ in range(nsteps):
         a = od.step(a, cfg["dt"])
         b = ob.step(b, cfg["dt"])
-    e, ep = rel_l2(b[:nf], a[:nf]), rel_l2_pert(b[:nf], a[:nf], cfg["K"])
-    print(f"cfg {ci + 1}: banded vs dense after {nsteps} steps: R14 {e:.2e}, without (0,0) {ep:.2e}")
-    assert e <= 1e-12
-    assert ep <= 1e-9
+        c = oc.step(c, cfg["dt"], workers=4)
+    for name, x in (("banded", b), ("c", c)):
+        e, ep = rel_l2(x[:nf], a[:nf]), rel_l2_pert(x[:nf], a[:nf], cfg["K"])
+        print(f"cfg {ci + 1}: {name} vs dense after {nsteps} steps: R14 {e:.2e}, without (0,0) {ep:.2e}")
+        assert e <= 1e-12
+        assert ep <= 1e-9
 
 
 def test_extended_precision_oracle_and_the_round_off_floor():
