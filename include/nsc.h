@@ -64,6 +64,9 @@ typedef struct nsc_params {
     int device;       /* CUDA device ordinal; -1 => current device                                */
     int radial_chunk; /* radial nodes per pass of the transform pipeline; 0 => automatic (all N_r
                        * at once when the work arrays fit an eighth of the device memory)         */
+    int linear_slices;/* mode slices of the implicit sub-step, each a chain of four sweep kernels on a
+                       * stream of its own; 0 => 2, at most 8                    */
+    int no_graph;     /* nonzero: nsc_step never captures / replays a CUDA graph (plain launches)     */
 } nsc_params;
 
 /* BJ: nsc_create(N_r, M_theta, K_z, eta, alpha, k_theta0, Re_i, Re_o, Ra, Pr, radial-grid type).

@@ -136,15 +136,9 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
     if (jc > c->N_r) jc = c->N_r;
     c->JC = jc;
 
-    // length-768 transform pipeline (nonlinear_v2.cuh); NSC_NL_VARIANT (experiments): bit 0 = z kernels,
-    // bits 1-2 = theta kernel (1 shared-memory scratch, 2 TMEM scratch); default 1 | 2 << 1
-    {
-        int variant = 1 | (2 << 1);
-        if (const char* ev = getenv("NSC_NL_VARIANT")) variant = atoi(ev);
-        c->z768 = (variant & 1) && c->Nz == 768 && c->K <= 256 && c->MP % 4 == 0;
-        c->t768 = (c->Nt == 768 && c->M <= 256 && c->nf == 3) ? ((variant >> 1) & 3) : 0;
-        if (c->t768 > 2) c->t768 = 2;
-    }
+    // length-768 transform pipeline (nonlinear_v2.cuh)
+    c->z768 = c->Nz == 768 && c->K <= 256 && c->MP % 4 == 0;
+    c->t768 = (c->Nt == 768 && c->M <= 256 && c->nf == 3) ? 2 : 0;
     int rc = build_plan(c);
     if (!rc && c->z768 && c->JC < c->N_r)     // D1 f arrays of the multi-chunk transform pipeline
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->DR[i], c->F, false);
@@ -159,8 +153,8 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
         if (!rc) rc = dev_alloc(c, &c->zbuf, (size_t)3 * c->nf * c->JC * c->Nz * c->MP, true);
         if (!rc) rc = dev_alloc(c, &c->tbuf, (size_t)c->nf * c->JC * c->Nz * c->MP, true);
     }
-    if (const char* ev = getenv("NSC_GRAPH")) c->use_graph = atoi(ev) != 0;
-    if (const char* ev = getenv("NSC_LIN_SLICES")) c->n_slices = atoi(ev);
+    c->use_graph = p.no_graph == 0;
+    c->n_slices = p.linear_slices > 0 ? p.linear_slices : 2;
     if (c->n_slices < 1) c->n_slices = 1;
     if (c->n_slices > NSC_MAX_SLICES) c->n_slices = NSC_MAX_SLICES;
     for (int i = 0; i < c->n_slices && !rc && c->n_slices > 1; ++i)

@@ -42,6 +42,7 @@ class nsc_params(C.Structure):
         ("Re_i", C.c_double), ("Re_o", C.c_double), ("Ra", C.c_double), ("Pr", C.c_double),
         ("radial_grid", C.c_int), ("n_theta_phys", C.c_int), ("n_z_phys", C.c_int),
         ("c", C.c_double), ("device", C.c_int), ("radial_chunk", C.c_int),
+        ("linear_slices", C.c_int), ("no_graph", C.c_int),
     ]
 
 
@@ -122,11 +123,11 @@ class Context:
     """One Taylor-Couette configuration on one GPU (``nsc_create`` ... ``nsc_destroy``)."""
 
     def __init__(self, N_r, M, K, eta, alpha, k_theta0, Re_i, Re_o, Ra=0.0, Pr=1.0, grid=1,
-                 n_theta=0, n_z=0, c=0.0, device=-1, radial_chunk=0):
+                 n_theta=0, n_z=0, c=0.0, device=-1, radial_chunk=0, linear_slices=0, no_graph=0):
         self._lib = load_library()
         self._h = C.c_void_p()
         p = nsc_params(N_r, M, K, eta, alpha, k_theta0, Re_i, Re_o, Ra, Pr, grid, n_theta, n_z, c,
-                       device, radial_chunk)
+                       device, radial_chunk, linear_slices, no_graph)
         rc = self._lib.nsc_create_ex(C.byref(self._h), C.byref(p))
         if rc != NSC_OK:
             msg = self._lib.nsc_last_error(None).decode()
