@@ -601,6 +601,87 @@ class Oracle:
                 break
         return cur, k, err
 
+    # ---------------------------------------------------------------- NEXT-1: dynamic step-size control
+    def radial_spacing(self):
+        """Delta r_j = the smaller of the two spacings next to node j (one-sided at the walls)."""
+        d = np.diff(self.r.astype(np.float64))
+        return np.minimum(np.concatenate([[d[0]], d]), np.concatenate([d, [d[-1]]]))
+
+    def cfl_rate(self, state):
+        """Advective CFL rate lambda (1 / time) of a state, the largest over the physical grid of
+            |u_r| / Delta r_j,   |u_theta| / (r_j Delta theta),   |u_z| / Delta z,
+        Delta theta = 2 pi / (k_theta0 N_theta), Delta z = 2 pi / (alpha N_z) (SURVEY.md S12's rule; R17): a step
+        of size dt has CFL number lambda dt.  Returns (lambda, per-component maxima [3][N_r])."""
+        p = self.p
+        dth = 2 * np.pi / (p.k_theta0 * p.n_theta)
+        dz = 2 * np.pi / (p.alpha * p.n_z)
+        mx = np.stack([np.abs(self.to_physical(f)).reshape(p.N_r, -1).max(axis=1) for f in state[:3]]).astype(np.float64)
+        r = self.r.astype(np.float64)
+        lam = max(float((mx[0] / self.radial_spacing()).max()), float((mx[1] / (r * dth)).max()), float((mx[2] / dz).max()))
+        return lam, mx
+
+    @staticmethod
+    def dt_grid_floor(x):
+        """Largest value (8 + i) / 8 * 2^e, i = 0..7, that is <= x: step sizes are kept on this geometric grid
+        (ratio ~1.09) so that a controller re-uses the factored per-mode matrices (R17)."""
+        m, e = np.frexp(x)                          # x = m 2^e, 0.5 <= m < 1
+        return float(np.ldexp(np.floor(m * 16) / 16, e))
+
+    @staticmethod
+    def dt_grid_next(x):
+        """The grid value above the grid value x."""
+        m, e = np.frexp(x)
+        return float(np.ldexp((np.floor(m * 16) + 1) / 16, e))
+
+    def advance(self, state, t_end, max_steps, dt0, tol, cfl, max_corr):
+        """Time integration with dynamic step-size control ("a variable time-step size with dynamic
+        control"; the paper's rule is in its ref. [6], not available: DESIGN.md reading R17).  From t = 0:
+            dt_cur <- grid_floor(dt0);  repeat until t = t_end or max_steps attempts:
+              lambda = cfl_rate(u^n);  dt = min(dt_cur, grid_floor(cfl / lambda), t_end - t)
+              (u, k, err) = step_iterated(u^n, dt, tol, max_corr)
+              err <= tol : accept, t += dt, dt_cur <- grid_next(dt) if k <= 2, err <= tol / 2 and dt == dt_cur, else kept
+              err >  tol : reject (state unchanged), dt_cur <- grid_floor(dt / 2)
+        Returns (state, t, log) with log = list of (dt, k, err, accepted)."""
+        t, log = 0.0, []
+        dt_cur = self.dt_grid_floor(dt0)
+        while t < t_end and len(log) < max_steps:
+            lam, _ = self.cfl_rate(state)
+            dt = dt_cur
+            if lam > 0.0:
+                dt = min(dt, self.dt_grid_floor(cfl / lam))
+            last = t_end - t <= dt
+            if last:
+                dt = t_end - t
+            new, k, err = self.step_iterated(state, dt, tol, max_corr)
+            ok = err <= tol
+            log.append((dt, k, err, ok))
+            if ok:
+                state = new
+                t = t_end if last else t + dt
+                if k <= 2 and err <= 0.5 * tol and dt == dt_cur:
+                    dt_cur = self.dt_grid_next(dt_cur)
+            else:
+                dt_cur = self.dt_grid_floor(dt / 2)
+        return state, t, log
+
+    # ---------------------------------------------------------------- NEXT-3: wave speed
+    def wave_speed(self, state, field, j, m, k, dt, n_steps):
+        """Angular phase speed of one Fourier coefficient f^(r_j; m, k) ~ e^{i (n theta - omega t)} over n_steps
+        plain steps of size dt (the CI validation compares "the wave speed of a simulated wavy
+        vortex flow" with an experiment): omega / n, n = m k_theta0 >= 1, with
+        omega = - sum_i arg(f_{i+1} conj f_i) / (n_steps dt)  (phase increments per step, each in (-pi, pi]).
+        Returns (speed, state after the steps)."""
+        n = m * self.p.k_theta0
+        kk = k + self.p.K
+        f0 = complex(state[field][j, m, kk])
+        dphi = 0.0
+        for _ in range(n_steps):
+            state = self.step(state, dt)
+            f1 = complex(state[field][j, m, kk])
+            dphi += float(np.angle(f1 * np.conj(f0)))
+            f0 = f1
+        return -dphi / (n_steps * dt) / n, state
+
     # ---------------------------------------------------------------- NEXT-3: diagnostics
     def nusselt(self, state):
         """Wall diagnostics of PAPER.md:100-108 (Fig. 3a plots Nu_i): transfer at a wall normalised by that of

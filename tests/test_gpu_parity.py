@@ -4,14 +4,28 @@ concatenated, base flow included) <= 1e-11 per nonlinear evaluation, <= 1e-9 aft
 import numpy as np
 import pytest
 
+import os
+
 from helpers import oracle_of, nf_of
-from oracle.nsc_oracle import rel_l2
+from oracle.nsc_oracle import rel_l2, rel_l2_pert
 from paper_1908_00587_b200 import synth
 
 pytestmark = pytest.mark.gpu
 
 TOL_N = 1e-11
 TOL_STEP = 1e-9
+NCPU = os.cpu_count() or 1
+
+
+def check_parity(got, ref, tol, K, what, mean_index="full"):
+    """Asserts the R14 norm (all fields, base flow included) against ``tol`` and the same norm with the mean
+    mode (0,0) left out (the base flow, 1e2..1e4 times the perturbation, sits there and would
+    discount an error confined to the perturbation modes) against 10 * ``tol``; prints both."""
+    e = rel_l2(got, ref)
+    ep = rel_l2_pert(got, ref, K) if mean_index == "full" else rel_l2_pert(got, ref, K, mean_index=mean_index)
+    print(f"{what}: rel-L2 {e:.2e}, without mode (0,0) {ep:.2e}")
+    assert e <= tol, (what, e)
+    assert ep <= 10 * tol, (what, "without (0,0)", ep)
 
 
 @pytest.fixture(scope="module")
@@ -49,11 +63,12 @@ NL_CASES = [
     (2, 11, 4, 16, "naive"),      # heated; lengths 12 / 48
     (1, 13, 32, 32, "naive"),     # lengths 96 / 96
     (2, 10, 64, 8, "naive"),      # heated; 192 / 24
-    (3, 9, 128, 4, "fft"),        # 384 / 12
-    (3, 12, 256, 8, "fft"),       # 768 / 24  (cfg 4's theta length)
-    (1, 10, 8, 256, "fft"),       # 24 / 768  (cfg 4's z length)
-    (4, 9, 512, 4, "fft"),        # heated; 1536 / 12 (cfg 5's theta length)
-    (4, 9, 4, 512, "fft"),        # heated; 12 / 1536
+    (3, 9, 128, 4, "naive"),      # 384 / 12
+    (3, 12, 256, 8, "naive"),     # 768 / 24  (cfg 4's theta length)
+    (1, 10, 8, 256, "naive"),     # 24 / 768  (cfg 4's z length)
+    (4, 9, 512, 4, "naive"),      # heated; 1536 / 12 (cfg 5's theta length)
+    (4, 9, 4, 512, "naive"),      # heated; 12 / 1536
+    (2, 10, 128, 128, "naive"),   # heated; 384 / 384 (cfg 3's lengths)
 ]
 
 
@@ -68,7 +83,36 @@ def test_nonlinear_matches_oracle(torch_cuda, ci, N_r, M, K, dft):
         ctx.set_state(*_dev(torch, st))
         got = ctx.nonlinear_to_host()
     ref = o.nonlinear(*st[:nf_of(cfg)])
-    assert rel_l2(got, ref) <= TOL_N
+    check_parity(got, ref, TOL_N, K, f"nonlinear {N_r}x{M}x{K}")
+
+
+@pytest.mark.parametrize("ci,N_r,M,K,n_theta,n_z", [(3, 9, 128, 8, 768, 0), (1, 9, 8, 128, 0, 768), (3, 10, 64, 64, 768, 768)])
+def test_nonlinear_length_768_kernels_on_a_padded_grid(torch_cuda, ci, N_r, M, K, n_theta, n_z):
+    """The length-768 kernels with fewer than 256 modes (a physical grid padded beyond the 3/2 rule through
+    n_theta_phys / n_z_phys = 768): more zero slots on input, fewer kept on output."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    o = oracle_of(cfg, dft="naive", n_theta=n_theta, n_z=n_z)
+    with _ctx(cfg, n_theta=n_theta, n_z=n_z) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        got = ctx.nonlinear_to_host()
+    check_parity(got, o.nonlinear(*st[:3]), TOL_N, K, f"nonlinear {N_r}x{M}x{K} on {n_theta or 3 * M} x {n_z or 3 * K}")
+
+
+@pytest.mark.parametrize("ci,N_r,M,K", [(3, 9, 256, 256), (2, 9, 128, 128)])
+def test_nonlinear_white_noise_through_the_long_transforms(torch_cuda, ci, N_r, M, K):
+    """Full-band white-noise fields with a non-Hermitian m = 0 row (reading R6) through the length-768 and
+    length-384 kernels, against the naive-DFT oracle."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    nf = nf_of(cfg)
+    o = oracle_of(cfg, dft="naive")
+    fs = _random_fields(cfg, 6, nf)
+    with _ctx(cfg) as ctx:
+        ctx.set_state(*(_dev(torch, fs) + [None] * (5 - nf)))
+        got = ctx.nonlinear_to_host()
+    check_parity(got, o.nonlinear(*fs), TOL_N, K, f"white-noise nonlinear {N_r}x{M}x{K}")
 
 
 def test_nonlinear_broadband_random_fields_and_chunking(torch_cuda):
@@ -142,7 +186,45 @@ def test_steps_match_oracle(torch_cuda, ci, N_r, M, K, nsteps):
     ref = st
     for _ in range(nsteps):
         ref = o.step(ref, cfg["dt"])
-    assert rel_l2(got[:nf], ref[:nf]) <= TOL_STEP
+    check_parity(got[:nf], ref[:nf], TOL_STEP, K, f"{nsteps} steps {N_r}x{M}x{K}")
+
+
+def _twenty_steps_full(torch, ci, side_stream):
+    """20 nsc_step calls at a full BASELINE.json configuration against 20 oracle steps (the north-star
+    criterion).  Oracle: library FFT (pinned to the naive sums at these lengths, tests/test_oracle_transforms.py)
+    and the plain-C banded elimination (pinned to the dense one, tests/test_oracle_banded.py)."""
+    cfg = synth.config(ci)
+    nf = nf_of(cfg)
+    o = oracle_of(cfg, dft="fft", solve="c")
+    with _ctx(cfg) as ctx:
+        if side_stream:                       # a non-default stream: the steps are CUDA-graph replays
+            s = torch.cuda.Stream()
+            ctx.set_stream(s)
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        for _ in range(20):
+            ctx.step(cfg["dt"])
+        got = ctx.state_to_host()
+        replays = ctx.graph_replays()
+    assert replays == (20 if side_stream else 0)
+    ref = st
+    for _ in range(20):
+        ref = o.step(ref, cfg["dt"], workers=NCPU)
+    check_parity(got[:nf], ref[:nf], TOL_STEP, cfg["K"], f"20 steps at full cfg {ci + 1}")
+
+
+@pytest.mark.parametrize("ci", [1, 2])
+def test_twenty_steps_at_full_size(torch_cuda, ci):
+    """BASELINE.json configs[1] (64 x 33 x 65 modes) and configs[2] (heated, 128 x 129 x 257 modes; the oracle
+    takes ~10 s per step on 16 cores)."""
+    _twenty_steps_full(torch_cuda, ci, side_stream=(ci == 2))
+
+
+@pytest.mark.skipif(not os.environ.get("NSC_TEST_CFG4_20STEPS"), reason="opt-in: the oracle takes ~2 min per step at cfg 4")
+def test_twenty_steps_at_full_cfg4(torch_cuda):
+    """BASELINE.json configs[3] (N_r = 256, 257 x 513 modes; bench.py's workload, graph replays on a side
+    stream).  Opt-in (NSC_TEST_CFG4_20STEPS=1); the last recorded figures are in DESIGN.md section 9."""
+    _twenty_steps_full(torch_cuda, 3, side_stream=True)
 
 
 def test_couette_flow_is_a_fixed_point_on_the_gpu(torch_cuda):
@@ -190,7 +272,7 @@ def test_full_size_sampled(torch_cuda, ci):
     cfg = synth.config(ci)
     nf = nf_of(cfg)
     N_r = cfg["N_r"]
-    o = oracle_of(cfg, dft="fft")
+    o = oracle_of(cfg, dft="naive")      # the naive sums decide at the sampled nodes; the sub-step uses no transform
     nodes = [0, 1, 4, N_r // 2 - 1, (3 * N_r) // 4, N_r - 5, N_r - 2, N_r - 1]
     rng = np.random.default_rng(11)
     im = np.concatenate([[0, 0, 0, cfg["M"], cfg["M"], 1], rng.integers(0, cfg["M"] + 1, 26)])
@@ -200,14 +282,15 @@ def test_full_size_sampled(torch_cuda, ci):
         ctx.set_state(*_dev(torch, st))
         got = ctx.nonlinear_to_host()
         ref = o.nonlinear(*st[:nf], nodes=nodes)
-        assert rel_l2([g[nodes] for g in got], ref) <= TOL_N
+        check_parity([g[nodes] for g in got], ref, TOL_N, cfg["K"], f"cfg {ci + 1} nonlinear at {len(nodes)} nodes")
         # sub-step with the nonlinear term just computed as the explicit term
         E = got
         ctx.substep(*(_dev(torch, E) + [None] * (4 - nf)), cfg["dt"])
         sub = ctx.state_to_host()
         ref_s = o.substep(st, E, cfg["dt"], modes=(im, ik))
         got_s = [f[:, im, ik] for f in sub[:nf]]
-        assert rel_l2(got_s, ref_s[:nf]) <= TOL_STEP
+        mean = np.nonzero((im == 0) & (ik == cfg["K"]))[0]
+        check_parity(got_s, ref_s[:nf], 1e-11, cfg["K"], f"cfg {ci + 1} sub-step at {len(im)} modes", mean_index=mean)
         # scaled divergence of the new state (formula of SURVEY.md section 8(c), pin T5)
         ur, ut, uz = sub[:3]
         r = o.r[:, None, None]
@@ -347,7 +430,7 @@ def test_nonlinear_length_768_in_several_radial_chunks(torch_cuda, ci, N_r, M, K
     the work arrays of the whole radius do not fit) against the oracle, and against the single-chunk form."""
     torch = torch_cuda
     cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
-    o = oracle_of(cfg, dft="fft")
+    o = oracle_of(cfg, dft="naive")
     res = []
     for rc in (chunk, 0):
         with _ctx(cfg, radial_chunk=rc) as ctx:
@@ -355,8 +438,8 @@ def test_nonlinear_length_768_in_several_radial_chunks(torch_cuda, ci, N_r, M, K
             ctx.set_state(*_dev(torch, st))
             res.append(ctx.nonlinear_to_host())
     ref = o.nonlinear(*st[:3])
-    assert rel_l2(res[0], ref) <= TOL_N
-    assert rel_l2(res[1], ref) <= TOL_N
+    check_parity(res[0], ref, TOL_N, K, "768 pipeline, several chunks")
+    check_parity(res[1], ref, TOL_N, K, "768 pipeline, one chunk")
     assert rel_l2(res[0], res[1]) <= 1e-13
 
 
@@ -370,9 +453,9 @@ def test_full_size_cfg5_sampled(torch_cuda):
     import os
     torch = torch_cuda
     cfg = synth.config(4)
-    o = oracle_of(cfg, dft="fft")
+    o = oracle_of(cfg, dft="naive")
     N_r = cfg["N_r"]
-    nodes = [0, 3, N_r // 2, N_r - 6, N_r - 1]
+    nodes = [0, N_r // 2 + 3, N_r - 1]
     with_substep = bool(os.environ.get("NSC_TEST_CFG5_SUBSTEP"))
     rng = np.random.default_rng(12)
     im = np.concatenate([[0, 0, cfg["M"], 1], rng.integers(0, cfg["M"] + 1, 12)])
@@ -382,9 +465,7 @@ def test_full_size_cfg5_sampled(torch_cuda):
         ctx.set_state(*st)
         E = ctx.nonlinear_to_host()
         ref = o.nonlinear(*st[:4], nodes=nodes)
-        err_n = rel_l2([g[nodes] for g in E], ref)
-        print("cfg 5 sampled: nonlinear rel-L2", err_n)
-        assert err_n <= TOL_N
+        check_parity([g[nodes] for g in E], ref, TOL_N, cfg["K"], "cfg 5 nonlinear at sampled nodes")
         if not with_substep:
             return
         ctx.substep(*_dev(torch, E), cfg["dt"])
@@ -424,7 +505,37 @@ def test_step_graph_replay_equals_plain_launches(torch_cuda):
             torch.cuda.synchronize()
             counts.append(ctx.launch_count() - n0)
             res.append(ctx.state_to_host())
+            assert ctx.graph_replays() == (6 if side else 0)     # every nsc_step on the side stream was a replay
     assert counts[0] == counts[1]
     for a, b in zip(*res):
         if a is not None:
+            np.testing.assert_array_equal(a, b)
+
+
+def test_graph_replay_after_a_substep_with_another_dt(torch_cuda):
+    """nsc_step(dt), nsc_substep(E, dt / 2), nsc_step(dt) on a side stream: the sub-step rebuilds the Helmholtz
+    factors in place for dt / 2, so the cached step graph must see factors for dt again before it is replayed.
+    Compared bit for bit with a context that never uses a graph (nsc_params.no_graph)."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(2, N_r=18, M=8, K=8)
+    nf = nf_of(cfg)
+    dt = cfg["dt"]
+    res = []
+    for no_graph in (1, 0):
+        with _ctx(cfg, no_graph=no_graph) as ctx:
+            s = torch.cuda.Stream()
+            ctx.set_stream(s)
+            st = synth.make_state(cfg, ctx.grid())
+            ctx.set_state(*_dev(torch, st))
+            E = _dev(torch, [1e3 * f for f in _random_fields(cfg, 2, nf)])
+            ctx.step(dt)
+            ctx.substep(*E, 0.5 * dt)
+            ctx.step(dt)
+            ctx.step(dt)
+            torch.cuda.synchronize()
+            assert ctx.graph_replays() == (0 if no_graph else 3)
+            res.append(ctx.state_to_host())
+    for a, b in zip(*res):
+        if a is not None:
+            assert np.isfinite(a).all()
             np.testing.assert_array_equal(a, b)
