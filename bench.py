@@ -82,15 +82,24 @@ def flops_per_nonlinear(cfg):
 
 LINEAR_KERNELS = ("k_rhs_fwd", "k_bwd_div", "k_poisson_fwd", "k_poisson_bwd_correct")
 
-# fp64 peak of the plain DFMA pipe: 148 SM x 64 lanes x 2 flop x 1.965 GHz
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# nominal fp64 peak of the plain DFMA pipe (context; the roofline uses the peaks measured by nsc_fp64_peak):
+# 148 SM x 64 lanes x 2 flop x 1.965 GHz
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r01_final_ncu_full.md), cfg 4, one launch = all 256 radial levels; None where no capture exists
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    ("k_theta", 4): 7.498633e9 + 2.536703e9,
-    ("k_zinv", 4): 1.620360e9 + 4.930793e9,
-}
+def ncu_traffic(kernel, config):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of ``kernel`` at BASELINE config ``config`` from the
+    committed `ncu --set full` capture (profiles/r02_ncu_traffic.csv: kernel, config, bytes per launch, capture), or
+    (None, None) if that kernel was not captured."""
+    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.csv")
+    try:
+        with open(path) as fh:
+            for line in fh:
+                parts = [p.strip() for p in line.split(",")]
+                if len(parts) >= 4 and parts[0] == kernel and parts[1] == str(config):
+                    return float(parts[2]), parts[3]
+    except OSError:
+        pass
+    return None, None
 
 
 def flops_theta_per_nonlinear(cfg):
@@ -253,6 +262,43 @@ def workload_name(cfg):
             f"Ra={cfg['Ra']:g}, temperature {'on' if s['nf'] == 4 else 'off'}")
 
 
+def time_extra_config(ci, args, stream):
+    """Device-resident steps/s of another BASELINE.json configuration in the same run (parity-test cases, not the
+    headline: 3 warm-up steps, then args.steps timed steps), with the per-kernel CUDA-event times."""
+    import torch
+    from paper_1908_00587_b200 import nsc, synth
+    cfg = synth.config(ci - 1)
+    cfg["index"] = ci - 1
+    model = algorithmic_bytes(cfg)
+    with nsc.Context.from_config(cfg) as ctx:
+        ctx.set_stream(stream)
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*st)
+        del st
+        for _ in range(3):
+            ctx.step(cfg["dt"])
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            ctx.step(cfg["dt"])
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        ctx.set_profiling(True)
+        ctx.profile_read()
+        for _ in range(args.steps):
+            ctx.step(cfg["dt"])
+        prof = ctx.profile_read()
+        ctx.set_profiling(False)
+        dev_bytes = ctx.device_bytes()
+    peak, _ = measured_peaks()
+    return {"workload": workload_name(cfg), "ms_per_step": ms, "steps_per_s": 1e3 / ms,
+            "step_algorithmic_GB": model["step"] / 1e9, "step_frac_of_measured_hbm": model["step"] / 1e6 / ms / peak,
+            "device_bytes": dev_bytes,
+            "kernels_ms_per_step": {n: k / args.steps for n, (k, c) in prof.items() if c and n != "k_factor"}}
+
+
 def run_ours(args, cfg, rank, world, local_rank):
     import torch
     from paper_1908_00587_b200 import build, nsc, synth, replicas
@@ -355,6 +401,14 @@ def run_ours(args, cfg, rank, world, local_rank):
         finite = bool(np.isfinite(host_out[1]).all())
         dev_bytes = ctx.device_bytes()
 
+    # ---- measured fp64 peaks of this device (register-only kernels, nsc_fp64_peak) and the other configurations
+    fp64_fma = nsc.fp64_peak(0)
+    fp64_addmul = nsc.fp64_peak(1)
+    extra = []
+    if rank == 0 and world == 1:
+        for ci in args.extra_configs:
+            extra.append(time_extra_config(ci, args, stream))
+
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
@@ -391,10 +445,16 @@ def run_ours(args, cfg, rank, world, local_rank):
     if dom is None or (lin_ms > dom["ms_per_step"]):
         dom = lin
     launches_dom = dom.get("launches_per_step", None)
+    traffic, traffic_src = ncu_traffic(dom["kernel"], args.config)
+    for k in kern:
+        k["bound"] = "fp64" if k["kernel"] == "k_theta" else "hbm"
     roofline = {
         "bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_GBs"], "peak": peak, "unit": "GB/s",
         "frac": dom["achieved_GBs"] / peak, "peak_source": peak_src,
-        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((dom["kernel"], args.config)),
+        "note": ("the dominant kernel's algorithmic bytes over its time against the HBM copy peak; that kernel (the fused "
+                 "theta transforms) is bound by the fp64 pipe, see 'alu'; the step-level HBM fraction is 'step'"
+                 if dom["kernel"] == "k_theta" else None),
+        "traffic": traffic, "traffic_source": traffic_src,
         "share_of_step": dom["share"],
         "algorithmic_bytes_per_launch": (model.get(dom["kernel"], model["linear"]) / launches_dom
                                          if launches_dom else None),
@@ -404,10 +464,16 @@ def run_ours(args, cfg, rank, world, local_rank):
                  "frac_of_nominal_8TBs": model["step"] / 1e6 / ms_per_step / NOMINAL_HBM_GBS},
         "fp64": {"GF_per_nonlinear": flops_per_nonlinear(cfg) / 1e9},
         # the theta kernel is co-bound by the plain fp64 pipe: its own ALU roofline
-        "alu": ({"kernel": "k_theta", "achieved": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"],
-                 "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                 "frac": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"] / FP64_PEAK_TFLOPS,
-                 "peak_source": "148 SM x 64 DFMA lanes x 2 x 1.965 GHz (nominal)"}
+        # the theta kernel is bound by the plain fp64 pipe: its flops (model: 5 N log2 N per complex transform, mostly
+        # additions and multiplications that do not fuse) against the measured DADD+DMUL rate and the DFMA rate
+        "alu": ({"bound": "fp64", "kernel": "k_theta",
+                 "achieved": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"],
+                 "peak": fp64_addmul, "unit": "TFLOP/s",
+                 "frac": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"] / fp64_addmul,
+                 "peak_source": "measured: nsc_fp64_peak(kind 1, DADD + DMUL alternating, 1 flop per instruction)",
+                 "peak_dfma": fp64_fma, "frac_of_dfma_peak": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"] / fp64_fma,
+                 "peak_dfma_source": "measured: nsc_fp64_peak(kind 0, DFMA only, 2 flop per instruction)",
+                 "nominal_dfma_peak": FP64_NOMINAL_TFLOPS}
                 if (th := next((k for k in kern if k["kernel"] == "k_theta"), None)) else None),
         "kernels": kern + [lin],
         "ms_per_step_with_event_brackets": ms_prof_per_step,
@@ -434,6 +500,7 @@ def run_ours(args, cfg, rank, world, local_rank):
                 "d2h_bytes_per_step": nbytes_state, "steps": ke,
                 "what": "nsc_set_state_host (pinned) + nsc_step + nsc_get_state_host per step"},
         "roofline": roofline,
+        "other_configs": extra,
     }
     if not args.no_cpu_baseline and world == 1:
         t_step, desc, threads = oracle_sample(cfg)
@@ -452,6 +519,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--radial-chunk", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extra-configs", type=lambda v: [int(x) for x in v.split(",") if x], default=[3],
+                    help="other BASELINE.json configs timed in the same run and reported under other_configs (default 3)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print(f"bench.py: note: warmup {args.warmup} < 3 breaks the timing rules", file=sys.stderr)

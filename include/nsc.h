@@ -129,6 +129,44 @@ int nsc_step(nsc_ctx* ctx, double dt);
  * (2 n_f + 2) more field-sized buffers. */
 int nsc_step_iterated(nsc_ctx* ctx, double dt, double tol, int max_corr, int* n_corr, double* err);
 
+/* CFL rate lambda of the current state (reading R17): the largest over the physical
+ * grid of |u_r| / dr_j, |u_theta| / (r_j dtheta), |u_z| / dz with dr_j = the smaller radial spacing next to node j,
+ * dtheta = 2 pi / (k_theta0 N_theta), dz = 2 pi / (alpha N_z); a step of size dt has CFL number lambda dt.  Runs
+ * one nonlinear evaluation (the theta kernel gathers the maxima per radial level).  *h_rate: HOST double.
+ * Synchronises the stream. */
+int nsc_cfl_rate(nsc_ctx* ctx, double* h_rate);
+
+/* Time integration with dynamic step-size control ("variable time-step size with dynamic control"; the
+ * paper's rule is in its ref. [6], not available: DESIGN.md reading R17).  From t = 0, until t = t_end or max_steps
+ * attempts:   dt = min(dt_cur, floor(cfl / lambda(u^n)), t_end - t);  the step of nsc_step_iterated(dt, tol, max_corr)
+ *   err <= tol : accepted, t += dt;  dt_cur <- next grid value if it took <= 2 passes, err <= tol / 2 and dt == dt_cur
+ *   err >  tol : rejected, the state is untouched, dt_cur <- floor(dt / 2), tried again (N(u^n) is not recomputed)
+ * with dt_cur starting at floor(dt0); floor / next refer to the grid (8 + i) / 16 * 2^e, i = 0..7, so that the factored
+ * per-mode matrices are re-used.  h_info (HOST, may be NULL) receives the summary; h_log (HOST, may be NULL, 4 max_steps
+ * doubles) one record (dt, passes, err, accepted 1/0) per attempt.  Synchronises the stream once per corrector pass
+ * and once per step (the norm and the maxima are read back). */
+typedef struct nsc_advance_info {
+    double t;             /* time reached (== t_end unless max_steps ran out)                       */
+    double dt_next;       /* the controller's current step size (pass it as dt0 to continue)        */
+    double dt_last, dt_min, dt_max;   /* of the accepted steps                                      */
+    double err_last;      /* corrector norm of the last attempt                                     */
+    double cfl_rate_last; /* lambda of the last state a step started from                           */
+    int accepted, rejected, passes;   /* steps accepted / rejected, corrector passes in total       */
+} nsc_advance_info;
+int nsc_advance(nsc_ctx* ctx, double t_end, int max_steps, double dt0, double tol, double cfl, int max_corr,
+                nsc_advance_info* h_info, double* h_log);
+
+/* One Fourier coefficient f^(r_j; m, k) of the current state (field: 0 u_r, 1 u_theta, 2 u_z, 3 T, 4 p), as
+ * (re, im) in h_re_im (HOST, 2 doubles).  Synchronises the stream. */
+int nsc_mode_coefficient(nsc_ctx* ctx, int field, int j, int m, int k, double* h_re_im);
+
+/* Angular phase speed of that coefficient over n_steps calls of nsc_step(dt) (the
+ * CI validation compares "the wave speed of a simulated wavy vortex flow" with an experiment): for
+ * f ~ e^{i (n theta - omega t)}, n = m k_theta0 >= 1,  *h_speed = omega / n with
+ * omega = - sum_i arg(f_{i+1} conj f_i) / (n_steps dt)  (phase increments per step, each in (-pi, pi]).
+ * The state advances by n_steps steps.  Synchronises the stream after every step. */
+int nsc_wave_speed(nsc_ctx* ctx, int field, int j, int m, int k, double dt, int n_steps, double* h_speed);
+
 /* Wall diagnostics of the current state (Fig. 3a): transfer at a wall
  * normalised by that of the basic state at the same parameters, from the mean mode (0,0):
  *   h_out[0], h_out[1]  heat-flux Nusselt number at the inner / outer wall, d_r T r ln(eta)  (nan if Ra = 0)

@@ -7,11 +7,13 @@
 #include <cstring>
 #include <new>
 #include <utility>
+#include <vector>
 #include "nsc_internal.h"
 
 namespace nsc {
 
 bool fft_length_supported(int n);
+int warp_na(int n, int modes);
 
 static thread_local std::string g_create_err;
 
@@ -136,11 +138,11 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
     if (jc > c->N_r) jc = c->N_r;
     c->JC = jc;
 
-    // length-768 transform pipeline (nonlinear_v2.cuh)
-    c->z768 = c->Nz == 768 && c->K <= 256 && c->MP % 4 == 0;
-    c->t768 = (c->Nt == 768 && c->M <= 256 && c->nf == 3) ? 2 : 0;
+    // warp-transform pipeline for the lengths 768 and 384 (nonlinear_v2.cuh)
+    c->z_na = warp_na(c->Nz, c->K);
+    c->t_na = warp_na(c->Nt, c->M);
     int rc = build_plan(c);
-    if (!rc && c->z768 && c->JC < c->N_r)     // D1 f arrays of the multi-chunk transform pipeline
+    if (!rc && c->z_na && c->JC < c->N_r)     // D1 f arrays of the multi-chunk transform pipeline
         for (int i = 0; i < c->nf && !rc; ++i) rc = dev_alloc(c, &c->DR[i], c->F, false);
     if (!rc) {
         for (int i = 0; i < 5 && !rc; ++i)
@@ -365,25 +367,28 @@ int nsc_step(nsc_ctx* c, double dt) {
     return step_body(c, dt);
 }
 
-int nsc_step_iterated(nsc_ctx* c, double dt, double tol, int max_corr, int* n_corr, double* err) {
-    if (!c) return NSC_EINVAL;
-    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_step_iterated before nsc_set_state");
-    if (!(dt > 0.0)) return fail(c, NSC_EINVAL, "nsc_step_iterated: dt must be > 0");
-    if (!(tol >= 0.0) || max_corr < 1) return fail(c, NSC_EINVAL, "nsc_step_iterated: tol must be >= 0 and max_corr >= 1");
+// ---- NEXT-1: iterated corrector (R16) and step-size control (R17)
+static int iter_alloc(nsc_ctx* c) {
+    if (c->it_acc) return NSC_OK;                        // first use: ping-pong iterates + pressure of a pass
     int rc;
-    if (!c->it_acc) {                                    // first use: ping-pong iterates + pressure of a pass
-        for (int i = 0; i < c->nf; ++i) {
-            if ((rc = dev_alloc(c, &c->itA[i], c->F, false))) return rc;
-            if ((rc = dev_alloc(c, &c->itB[i], c->F, false))) return rc;
-        }
-        if ((rc = dev_alloc(c, &c->itP, c->F, false))) return rc;
-        if ((rc = dev_alloc(c, &c->itDP, c->F, false))) return rc;
-        cd* acc = nullptr;
-        if ((rc = dev_alloc(c, &acc, 1, true))) return rc;   // one complex = two doubles
-        c->it_acc = reinterpret_cast<double*>(acc);
+    for (int i = 0; i < c->nf; ++i) {
+        if ((rc = dev_alloc(c, &c->itA[i], c->F, false))) return rc;
+        if ((rc = dev_alloc(c, &c->itB[i], c->F, false))) return rc;
     }
+    if ((rc = dev_alloc(c, &c->itP, c->F, false))) return rc;
+    if ((rc = dev_alloc(c, &c->itDP, c->F, false))) return rc;
+    cd* acc = nullptr;
+    if ((rc = dev_alloc(c, &acc, 1, true))) return rc;   // one complex = two doubles
+    c->it_acc = reinterpret_cast<double*>(acc);
+    return NSC_OK;
+}
+
+// Predictor and up to max_corr corrector passes from the state, which is left untouched: the newest iterate ends
+// in itA, the pressure of its pass in itP / itDP.  have_N0: N0 = N(u^n) is already in c->N0.
+static int iterated_core(nsc_ctx* c, double dt, double tol, int max_corr, bool have_N0, int* k_out, double* e_out) {
+    int rc;
     // N0 = N(u^n);  u^(1) = substep(N0) -> itA (its pressure is discarded)
-    if ((rc = launch_nonlinear(c, c->state, c->N0))) return rc;
+    if (!have_N0 && (rc = launch_nonlinear(c, c->state, c->N0))) return rc;
     if ((rc = launch_substep(c, c->N0, 1.0, nullptr, 0.0, dt, c->itA, nullptr))) return rc;
     int k = 0;
     double e = 0.0;
@@ -400,13 +405,167 @@ int nsc_step_iterated(nsc_ctx* c, double dt, double tol, int max_corr, int* n_co
         for (int i = 0; i < c->nf; ++i) std::swap(c->itA[i], c->itB[i]);       // itA = newest iterate
         if (e <= tol) break;
     }
-    // accept: the newest iterate and the pressure of its pass become the state (pointer swaps, no copies)
+    *k_out = k;
+    *e_out = e;
+    return NSC_OK;
+}
+
+// accept: the newest iterate and the pressure of its pass become the state (pointer swaps, no copies)
+static void iterated_commit(nsc_ctx* c) {
     for (int i = 0; i < c->nf; ++i) std::swap(c->state[i], c->itA[i]);
     std::swap(c->state[4], c->itP);
     std::swap(c->DP, c->itDP);
     c->ptr_gen += 1;                                     // a captured step graph holds the old pointers
+}
+
+int nsc_step_iterated(nsc_ctx* c, double dt, double tol, int max_corr, int* n_corr, double* err) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_step_iterated before nsc_set_state");
+    if (!(dt > 0.0)) return fail(c, NSC_EINVAL, "nsc_step_iterated: dt must be > 0");
+    if (!(tol >= 0.0) || max_corr < 1) return fail(c, NSC_EINVAL, "nsc_step_iterated: tol must be >= 0 and max_corr >= 1");
+    int rc, k = 0;
+    double e = 0.0;
+    if ((rc = iter_alloc(c))) return rc;
+    if ((rc = iterated_core(c, dt, tol, max_corr, false, &k, &e))) return rc;
+    iterated_commit(c);
     if (n_corr) *n_corr = k;
     if (err) *err = e;
+    return NSC_OK;
+}
+
+// step sizes live on the geometric grid (8 + i) / 16 * 2^e, i = 0..7 (R17): the per-mode factors are re-used
+static double dt_grid_floor(double x) {
+    int e = 0;
+    const double m = frexp(x, &e);                       // x = m 2^e, 0.5 <= m < 1
+    return ldexp(floor(m * 16.0) / 16.0, e);
+}
+static double dt_grid_next(double x) {
+    int e = 0;
+    const double m = frexp(x, &e);
+    return ldexp((floor(m * 16.0) + 1.0) / 16.0, e);
+}
+
+// N0 = N(u^n) with the per-level maxima of |u| gathered by the theta kernel; *rate = the CFL rate lambda (R17)
+static int nonlinear_with_cfl(nsc_ctx* c, double* rate) {
+    int rc;
+    if (!c->cfl_max) {
+        cd* p = nullptr;
+        if ((rc = dev_alloc(c, &p, ((size_t)3 * c->N_r + 1) / 2, true))) return rc;     // 3 N_r 64-bit words
+        c->cfl_max = reinterpret_cast<unsigned long long*>(p);
+    }
+    NSC_CUDA(c, cudaMemsetAsync(c->cfl_max, 0, sizeof(unsigned long long) * 3 * c->N_r, c->stream));
+    c->want_cfl = true;
+    rc = launch_nonlinear(c, c->state, c->N0);
+    c->want_cfl = false;
+    if (rc) return rc;
+    std::vector<double> mx((size_t)3 * c->N_r);          // the bit patterns are those of non-negative doubles
+    NSC_CUDA(c, cudaMemcpyAsync(mx.data(), c->cfl_max, sizeof(double) * mx.size(), cudaMemcpyDeviceToHost, c->stream));
+    NSC_CUDA(c, cudaStreamSynchronize(c->stream));
+    const int N = c->N_r;
+    const double dth = 2.0 * M_PI / ((double)c->p.k_theta0 * (double)c->Nt);
+    const double dz = 2.0 * M_PI / (c->p.alpha * (double)c->Nz);
+    double lr = 0.0, lt = 0.0, lz = 0.0;
+    for (int j = 0; j < N; ++j) {
+        const double dl = c->r[j > 0 ? j : 1] - c->r[j > 0 ? j - 1 : 0];
+        const double dr = c->r[j < N - 1 ? j + 1 : N - 1] - c->r[j < N - 1 ? j : N - 2];
+        lr = fmax(lr, mx[3 * j] / fmin(dl, dr));
+        lt = fmax(lt, mx[3 * j + 1] / (c->r[j] * dth));
+        lz = fmax(lz, mx[3 * j + 2] / dz);
+    }
+    *rate = fmax(lr, fmax(lt, lz));
+    return NSC_OK;
+}
+
+int nsc_cfl_rate(nsc_ctx* c, double* h_rate) {
+    if (!c || !h_rate) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_cfl_rate before nsc_set_state");
+    return nonlinear_with_cfl(c, h_rate);
+}
+
+int nsc_advance(nsc_ctx* c, double t_end, int max_steps, double dt0, double tol, double cfl, int max_corr,
+                nsc_advance_info* h_info, double* h_log) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_advance before nsc_set_state");
+    if (!(t_end > 0.0) || max_steps < 1 || !(dt0 > 0.0) || !(tol >= 0.0) || !(cfl > 0.0) || max_corr < 1)
+        return fail(c, NSC_EINVAL, "nsc_advance: t_end, dt0, cfl must be > 0, tol >= 0, max_steps and max_corr >= 1");
+    int rc;
+    if ((rc = iter_alloc(c))) return rc;
+    nsc_advance_info info;
+    memset(&info, 0, sizeof(info));
+    double t = 0.0, dt_cur = dt_grid_floor(dt0), lam = 0.0;
+    bool have_N0 = false;
+    int n = 0;
+    while (t < t_end && n < max_steps) {
+        if (!have_N0) {
+            if ((rc = nonlinear_with_cfl(c, &lam))) return rc;
+            have_N0 = true;
+        }
+        double dt = dt_cur;
+        if (lam > 0.0) dt = fmin(dt, dt_grid_floor(cfl / lam));
+        const bool last = t_end - t <= dt;
+        if (last) dt = t_end - t;
+        int k = 0;
+        double e = 0.0;
+        if ((rc = iterated_core(c, dt, tol, max_corr, true, &k, &e))) return rc;
+        const bool ok = e <= tol;
+        if (h_log) {
+            h_log[4 * n] = dt;
+            h_log[4 * n + 1] = (double)k;
+            h_log[4 * n + 2] = e;
+            h_log[4 * n + 3] = ok ? 1.0 : 0.0;
+        }
+        ++n;
+        info.passes += k;
+        info.err_last = e;
+        info.cfl_rate_last = lam;
+        if (ok) {
+            iterated_commit(c);
+            have_N0 = false;                             // N0 belongs to the old state
+            t = last ? t_end : t + dt;
+            info.accepted += 1;
+            info.dt_last = dt;
+            if (info.dt_min == 0.0 || dt < info.dt_min) info.dt_min = dt;
+            if (dt > info.dt_max) info.dt_max = dt;
+            if (k <= 2 && e <= 0.5 * tol && dt == dt_cur) dt_cur = dt_grid_next(dt_cur);
+        } else {
+            info.rejected += 1;
+            dt_cur = dt_grid_floor(dt / 2.0);            // the state and N0 are untouched: try again
+        }
+    }
+    info.t = t;
+    info.dt_next = dt_cur;
+    if (h_info) *h_info = info;
+    return NSC_OK;
+}
+
+// ---- NEXT-3: wave speed
+int nsc_mode_coefficient(nsc_ctx* c, int field, int j, int m, int k, double* h_re_im) {
+    if (!c || !h_re_im) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_mode_coefficient before nsc_set_state");
+    if (field < 0 || field > 4 || (field == 3 && !c->heated) || j < 0 || j >= c->N_r || m < 0 || m > c->M || k < -c->K || k > c->K)
+        return fail(c, NSC_EINVAL, "nsc_mode_coefficient: field 0..4 (3 only with temperature), 0 <= j < N_r, 0 <= m <= M, |k| <= K");
+    const size_t off = ((size_t)j * c->M1 + m) * c->NK + (size_t)(k + c->K);
+    NSC_CUDA(c, cudaMemcpyAsync(h_re_im, c->state[field] + off, sizeof(cd), cudaMemcpyDeviceToHost, c->stream));
+    NSC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NSC_OK;
+}
+
+int nsc_wave_speed(nsc_ctx* c, int field, int j, int m, int k, double dt, int n_steps, double* h_speed) {
+    if (!c || !h_speed) return NSC_EINVAL;
+    if (m < 1 || n_steps < 1) return fail(c, NSC_EINVAL, "nsc_wave_speed: m must be >= 1 and n_steps >= 1");
+    double f0[2], f1[2];
+    int rc = nsc_mode_coefficient(c, field, j, m, k, f0);
+    if (rc) return rc;
+    double dphi = 0.0;
+    for (int i = 0; i < n_steps; ++i) {
+        if ((rc = nsc_step(c, dt))) return rc;
+        if ((rc = nsc_mode_coefficient(c, field, j, m, k, f1))) return rc;
+        // arg(f1 conj(f0)), in (-pi, pi]
+        dphi += atan2(f1[1] * f0[0] - f1[0] * f0[1], f1[0] * f0[0] + f1[1] * f0[1]);
+        f0[0] = f1[0];
+        f0[1] = f1[1];
+    }
+    *h_speed = -dphi / ((double)n_steps * dt) / ((double)m * (double)c->p.k_theta0);
     return NSC_OK;
 }
 

@@ -1,43 +1,53 @@
-// fft768.cuh -- two-pass fp64 FFT of length 768 = 24 x 32 for one warp per line.
+// fft_warp.cuh -- two-pass fp64 FFTs of length N = NA x 32 (NA = 24: N = 768, NA = 12: N = 384) for one warp.
 //
-// The headline workload (BASELINE.json configs[3]: 768 x 768 physical grid per radial node) spends
-// its time in length-768 transforms.  With 24 complex values per thread the
-// generic three-pass plan of fft.cuh exchanges every line twice through shared memory and is bound
-// by the shared-memory crossbar (128 B/clk/SM), not by the DFMA pipe.  Here a line crosses shared
-// memory ONCE:
+// The long workloads (BASELINE.json configs[3]: 768 x 768 physical grid per radial node, configs[2]: 384 x 384)
+// spend their time in these transforms.  With 24 complex values per thread the generic
+// three-pass plan of fft.cuh exchanges every line twice through shared memory and is bound by the shared-memory
+// crossbar (128 B/clk/SM), not by the DFMA pipe.  Here a line crosses shared memory ONCE, and a warp always
+// carries 24 x 32 values: one line of 768 or LPW = 2 lines of 384.
 //
-//   "S" (spectral-side) layout : 32 lanes x 24 values, lane tau holds line index tau + 32 t, t < 24
-//   "P" (physical-side) layout : 24 lanes x 32 values, lane a   holds line index a + 24 p(e), e < 32,
-//                                p(e) = (e >> 3) + 4 (e & 7)   (register order left by the radix-32
-//                                butterfly; a static permutation, never materialised)
+//   "S" (spectral-side) layout : 32 lanes x 24 values; register t of lane tau holds index tau + 32 (t % NA) of
+//                                line t / NA
+//   "P" (physical-side) layout : 24 lanes x 32 values; lane a holds line a / NA, register e holds index
+//                                (a % NA) + NA p(e),  p(e) = (e >> 3) + 4 (e & 7)  (register order left by the
+//                                radix-32 butterfly; a static permutation, never materialised)
 //
-//   s2p :  S -> P     n = 32 n1 + tau,  k = a + 24 k2
-//          pass A  lane tau: DFT-24 over n1 (Good-Thomas 3 x 8, no inner twiddles), times W_768^(tau k1)
-//          exchange through a [24][33] complex matrix (row = k1 = a, column = tau; stride 33 keeps
+//   s2p :  S -> P     n = 32 n1 + tau,  k = k1 + NA k2
+//          pass A  lane tau: DFT-NA over n1 per line (Good-Thomas 3 x 2^q, no inner twiddles), times W_N^(tau k1)
+//          exchange through a [24][33] complex matrix (row = (line, k1) = a, column = tau; stride 33 keeps
 //          both the column-wise 16-byte stores and the row-wise 16-byte loads conflict free)
 //          pass B  lane a < 24: DFT-32 over tau (4 x 8 with W_32 constants)
-//   p2s :  P -> S     n = a + 24 n2,  k = 32 k1 + tau      (the mirror image)
+//   p2s :  P -> S     n = k1 + NA n2,  k = 32 k1' + tau      (the mirror image)
 //
-// Lanes 24..31 idle through the radix-32 halves (they recompute lane 23's butterfly and store
-// nothing), which costs DFMA issue slots only while the crossbar, the actual bound, moves no byte
-// for them.  X[k] = sum_n x[n] exp(DIR 2 pi i n k / 768), unnormalised.
+// Lanes 24..31 idle through the radix-32 halves (they recompute lane 23's butterfly and store nothing).
+// X[k] = sum_n x[n] exp(DIR 2 pi i n k / N), unnormalised.
 #pragma once
 #include "fft.cuh"
 
 namespace nsc {
-namespace f768 {
+namespace fw {
 
-constexpr int N = 768;
-constexpr int NA = 24;            // radix of the pass on the S side
-constexpr int NB = 32;            // radix of the pass on the P side
+constexpr int NB = 32;            // radix of the pass on the P side = lanes on the S side
+constexpr int NV = 24;            // values per lane on the S side = lanes on the P side
 constexpr int XS = 33;            // row stride (complex) of the exchange matrix and the twiddle table
-constexpr int XBUF = NA * XS;     // complex elements of one exchange matrix (12 672 bytes)
+constexpr int XBUF = NV * XS;     // complex elements of one exchange matrix (12 672 bytes)
 
-// physical line index of register e of lane a in the P layout
 NSC_HD int p_of(int e) { return (e >> 3) + 4 * (e & 7); }
-NSC_HD int p_idx(int e, int a) { return a + NA * p_of(e); }
-// line index of register t of lane tau in the S layout
-NSC_HD int s_idx(int t, int tau) { return tau + NB * t; }
+
+template <int NA_> struct WGeo {
+    static constexpr int NA = NA_;            // radix of the pass on the S side
+    static constexpr int N = NA * NB;         // line length
+    static constexpr int LPW = NV / NA;       // lines per warp
+    static constexpr int NMAX = N / 3;        // largest mode count of the 3/2 rule
+    // index within its line of register e of lane a (P layout), of register t of lane tau (S layout)
+    static NSC_HD int p_idx(int e, int a) { return (a % NA) + NA * p_of(e); }
+    static NSC_HD int s_idx(int t, int tau) { return tau + NB * (t % NA); }
+    // S-layout slot tt = t % NA can hold a non-zero spectral bin when the mode count is <= NMAX:
+    // bins 0..NMAX (tt <= NMAX / 32) and bins N - NMAX..N - 1 (tt >= NA - NMAX / 32)
+    static NSC_HD bool slot_pos(int tt) { return tt <= NMAX / NB; }
+    static NSC_HD bool slot_neg(int tt) { return tt >= NA - NMAX / NB; }
+    static NSC_HD bool slot_live(int tt) { return slot_pos(tt) || slot_neg(tt); }
+};
 
 // cos / sin of 2 pi e / 32, correctly rounded
 #ifdef __CUDACC__
@@ -123,20 +133,27 @@ template <int DIR> NSC_HD void dft32_perm_in(cd* x) {
     for (int kb = 0; kb < 8; ++kb) dft4<DIR>(x[kb], x[kb + 8], x[kb + 16], x[kb + 24]);
 }
 
-// ---------------------------------------------------------------- phases of the two transforms
-// tw[k1 * XS + n2] = exp(-2 pi i k1 n2 / 768), k1 < 24, n2 < 32
-
-// s2p, lane tau < 32: x[0..23] (S layout) -> DFT-24, twiddle, store column tau of the matrix
-template <int DIR> NSC_HD void s2p_front(cd* x, cd* buf, const cd* tw, int tau) {
-    Dft<24, DIR>::run(x);
+// the LPW transforms of length NA of the S side, in place
+template <int NA, int DIR> NSC_HD void dft_s(cd* x) {
 #pragma unroll
-    for (int k1 = 1; k1 < NA; ++k1) {
-        cd w = tw[k1 * XS + tau];
+    for (int l = 0; l < NV / NA; ++l) Dft<NA, DIR>::run(x + NA * l);
+}
+
+// ---------------------------------------------------------------- phases of the two transforms
+// tw[t * XS + n2] = exp(-2 pi i (t % NA) n2 / N), t < 24, n2 < 32  (plan.cu: one table per length)
+
+// s2p, lane tau < 32: x[0..23] (S layout) -> DFT-NA, twiddle, store column tau of the matrix
+template <int NA, int DIR> NSC_HD void s2p_front(cd* x, cd* buf, const cd* tw, int tau) {
+    dft_s<NA, DIR>(x);
+#pragma unroll
+    for (int t = 1; t < NV; ++t) {
+        if (t % NA == 0) continue;
+        cd w = tw[t * XS + tau];
         if (DIR > 0) w = conj(w);
-        x[k1] = x[k1] * w;
+        x[t] = x[t] * w;
     }
 #pragma unroll
-    for (int k1 = 0; k1 < NA; ++k1) buf[k1 * XS + tau] = x[k1];
+    for (int t = 0; t < NV; ++t) buf[t * XS + tau] = x[t];
 }
 // s2p, lane a < 24 (callers pass a = min(tau, 23)): load row a, DFT-32 -> x[0..31] (P layout)
 template <int DIR> NSC_HD void s2p_back(cd* x, const cd* buf, int a) {
@@ -158,26 +175,26 @@ template <int DIR> NSC_HD void p2s_front(cd* x, cd* buf, const cd* tw, int a, bo
 #pragma unroll
         for (int k2 = 0; k2 < NB; ++k2) buf[a * XS + k2] = x[k2];
 }
-// p2s, lane tau < 32: load column tau, DFT-24 -> x[0..23] (S layout)
-template <int DIR> NSC_HD void p2s_back(cd* x, const cd* buf, int tau) {
+// p2s, lane tau < 32: load column tau, DFT-NA -> x[0..23] (S layout)
+template <int NA, int DIR> NSC_HD void p2s_back(cd* x, const cd* buf, int tau) {
 #pragma unroll
-    for (int aa = 0; aa < NA; ++aa) x[aa] = buf[aa * XS + tau];
-    Dft<24, DIR>::run(x);
+    for (int t = 0; t < NV; ++t) x[t] = buf[t * XS + tau];
+    dft_s<NA, DIR>(x);
 }
 
 #ifdef __CUDACC__
 // Whole transforms for one warp; x has 32 elements.  `buf` is the warp's private exchange matrix.
-template <int DIR> __device__ __forceinline__ void s2p(cd* x, cd* buf, const cd* tw, int tau) {
+template <int NA, int DIR> __device__ __forceinline__ void s2p(cd* x, cd* buf, const cd* tw, int tau) {
     __syncwarp();                      // every lane has finished reading buf (previous transform)
-    s2p_front<DIR>(x, buf, tw, tau);
+    s2p_front<NA, DIR>(x, buf, tw, tau);
     __syncwarp();
-    s2p_back<DIR>(x, buf, tau < NA ? tau : NA - 1);
+    s2p_back<DIR>(x, buf, tau < NV ? tau : NV - 1);
 }
-template <int DIR> __device__ __forceinline__ void p2s(cd* x, cd* buf, const cd* tw, int tau) {
+template <int NA, int DIR> __device__ __forceinline__ void p2s(cd* x, cd* buf, const cd* tw, int tau) {
     __syncwarp();
-    p2s_front<DIR>(x, buf, tw, tau < NA ? tau : NA - 1, tau < NA);
+    p2s_front<DIR>(x, buf, tw, tau < NV ? tau : NV - 1, tau < NV);
     __syncwarp();
-    p2s_back<DIR>(x, buf, tau);
+    p2s_back<NA, DIR>(x, buf, tau);
 }
 
 // cooperative copy of the [24][33] twiddle matrix (global, plan.cu) into shared memory
@@ -186,5 +203,5 @@ __device__ __forceinline__ void load_twiddles(cd* tw_s, const cd* tw_g) {
 }
 #endif
 
-}  // namespace f768
+}  // namespace fw
 }  // namespace nsc

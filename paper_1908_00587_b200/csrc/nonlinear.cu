@@ -63,15 +63,17 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
     a.nf = c->nf;
     a.scale = 1.0 / ((double)c->Nt * (double)c->Nz);
     a.buoy = c->heated ? c->p.Ra / c->p.Pr : 0.0;
+    a.cfl = c->want_cfl ? c->cfl_max : nullptr;
     Nl2Args a2{};
-    a2.tw768 = c->t.tw768;
+    a2.tw_z = c->t.tw_wz;
+    a2.tw_t = c->t.tw_wt;
     a2.alpha = c->p.alpha;
     a2.ktheta0 = (double)c->p.k_theta0;
     // N1, radial derivative.  One radial chunk (JC = N_r): D1 is applied to the z-transformed fields inside the
     // work array after k_zinv (two transforms per line instead of three; D1 commutes with the z transform).
     // Several chunks: D1 f of every spectral field once per evaluation, transformed as a third line.
-    const bool dr_after_z = c->z768 && c->JC == c->N_r;
-    if (c->z768 && !dr_after_z) {
+    const bool dr_after_z = c->z_na && c->JC == c->N_r;
+    if (c->z_na && !dr_after_z) {
         DrArgs d{};
         for (int i = 0; i < c->nf; ++i) {
             d.f[i] = f[i];
@@ -91,10 +93,10 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
         a.nj = (c->N_r - j0 < c->JC) ? c->N_r - j0 : c->JC;
         a.tw = c->t.tw_z;
         prof_begin(c, NSC_K_ZINV);
-        if (c->z768) {
+        if (c->z_na) {
             a2.b = a;
-            a2.nitems = c->nf * a.nj * (c->MP / 4);
-            if (int e = launch_zinv2(a2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zinv2 launch");
+            a2.nitems = c->nf * a.nj * (c->MP / warp_mtile(c->z_na));
+            if (int e = launch_zinv2(c->z_na, a2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zinv2 launch");
         } else if (int e = lz->zinv(a, c->stream)) {
             return cuda_fail(c, (cudaError_t)e, "k_zinv launch");
         }
@@ -116,20 +118,20 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
         }
         a.tw = c->t.tw_t;
         prof_begin(c, NSC_K_THETA);
-        if (c->t768) {
+        if (c->t_na) {
             a2.b = a;
             a2.nitems = a.nj * a.Nz;
-            if (int e = launch_theta2(a2, c->t768 == 2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_theta2 launch");
+            if (int e = launch_theta2(c->t_na, a2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_theta2 launch");
         } else if (int e = lt->theta(a, c->stream)) {
             return cuda_fail(c, (cudaError_t)e, "k_theta launch");
         }
         prof_end(c);
         a.tw = c->t.tw_z;
         prof_begin(c, NSC_K_ZFWD);
-        if (c->z768) {
+        if (c->z_na) {
             a2.b = a;
-            a2.nitems = c->nf * a.nj * (c->MP / 4);
-            if (int e = launch_zfwd2(a2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zfwd2 launch");
+            a2.nitems = c->nf * a.nj * (c->MP / warp_mtile(c->z_na));
+            if (int e = launch_zfwd2(c->z_na, a2, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_zfwd2 launch");
         } else if (int e = lz->zfwd(a, c->stream)) {
             return cuda_fail(c, (cudaError_t)e, "k_zfwd launch");
         }

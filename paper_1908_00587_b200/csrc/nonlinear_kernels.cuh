@@ -30,7 +30,20 @@ struct NlArgs {
     const cd* tw;          // twiddles of the transform length of the kernel
     int N_r, M1, NK, K, M, MP, JC, Nz, j0, nj, nf;
     double scale, buoy;
+    unsigned long long* cfl;   // [N_r][3] running maxima of |u_r|, |u_theta|, |u_z| per radial level, as the ordered
+                           // bit patterns of non-negative doubles (theta kernels, atomicMax); null: not wanted
 };
+
+// largest of v >= 0 over the TPL threads of a line (a whole warp if TPL >= 32), merged into *dst by atomicMax
+template <int TPL> __device__ __forceinline__ void line_atomic_max(unsigned long long* dst, double v, int tau) {
+    unsigned long long b = (unsigned long long)__double_as_longlong(v);
+#pragma unroll
+    for (int o = (TPL < 32 ? TPL : 32) / 2; o > 0; o >>= 1) {
+        const unsigned long long c = __shfl_xor_sync(0xffffffffu, b, o);
+        b = c > b ? c : b;
+    }
+    if ((TPL >= 32 ? (int)(threadIdx.x & 31) : tau) == 0) atomicMax(dst, b);
+}
 
 // ------------------------------------------------------------------------------------------
 template <int NZ> struct ZCfg {
@@ -284,9 +297,25 @@ __global__ void __launch_bounds__(TCfg<NT>::THREADS) k_theta(NlArgs a) {
         UB(0, e) = x[e].x;
         UB(1, e) = x[e].y;
     }
+    if (a.cfl) {                                           // per-level maxima for the CFL rate (step-size control)
+        double m0 = 0.0, m1 = 0.0;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            m0 = fmax(m0, fabs(x[e].x));
+            m1 = fmax(m1, fabs(x[e].y));
+        }
+        line_atomic_max<TPL>(a.cfl + 3 * (a.j0 + jl), m0, tau);
+        line_atomic_max<TPL>(a.cfl + 3 * (a.j0 + jl) + 1, m1, tau);
+    }
     // P1: (u_z, d_r u_r)
     load_pair<NT>(x, LINE_A(2), false, LINE_C(0), false, a.nm, M, tau);
     fft_line<NT, +1>(x, buf, tw, tau);
+    if (a.cfl) {
+        double m2 = 0.0;
+#pragma unroll
+        for (int e = 0; e < E; ++e) m2 = fmax(m2, fabs(x[e].x));
+        line_atomic_max<TPL>(a.cfl + 3 * (a.j0 + jl) + 2, m2, tau);
+    }
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         UB(2, e) = x[e].x;

@@ -1,4 +1,4 @@
-// nonlinear_v2.cu -- instantiation and launchers of the length-768 transform kernels
+// nonlinear_v2.cu -- instantiation and launchers of the warp-transform kernels for the lengths 768 and 384
 // (nonlinear_v2.cuh).  Persistent grids sized from the SM count (148 on a B200).
 #include "nonlinear_v2.cuh"
 
@@ -26,38 +26,53 @@ int launch_dr(const DrArgs& a, int nf, cudaStream_t st) {
     return (int)cudaGetLastError();
 }
 
-int launch_zinv2(const Nl2Args& a, cudaStream_t st) {
-    if (int e = set_smem(k_zinv2, Z2_SMEM_INV)) return e;
+int warp_na(int n, int modes) {
+    if (n == 768 && modes <= 256) return 24;
+    if (n == 384 && modes <= 128) return 12;
+    return 0;
+}
+
+int warp_mtile(int na) { return na == 24 ? Z2Cfg<24>::MT : Z2Cfg<12>::MT; }
+
+template <int NA> static int launch_zinv2_t(const Nl2Args& a, cudaStream_t st) {
+    using C = Z2Cfg<NA>;
+    if (int e = set_smem(k_zinv2<NA>, C::SMEM_INV)) return e;
     int grid = 2 * sm_count();
     if (grid > a.nitems) grid = a.nitems;
-    k_zinv2<<<grid, Z2_THREADS, Z2_SMEM_INV, st>>>(a);
+    k_zinv2<NA><<<grid, Z2_THREADS, C::SMEM_INV, st>>>(a);
     return (int)cudaGetLastError();
 }
 
-int launch_zfwd2(const Nl2Args& a, cudaStream_t st) {
-    if (int e = set_smem(k_zfwd2, Z2_SMEM_FWD)) return e;
+template <int NA> static int launch_zfwd2_t(const Nl2Args& a, cudaStream_t st) {
+    using C = Z2Cfg<NA>;
+    if (int e = set_smem(k_zfwd2<NA>, C::SMEM_FWD)) return e;
     int grid = 2 * sm_count();
     if (grid > a.nitems) grid = a.nitems;
-    k_zfwd2<<<grid, Z2_THREADS, Z2_SMEM_FWD, st>>>(a);
+    k_zfwd2<NA><<<grid, Z2_THREADS, C::SMEM_FWD, st>>>(a);
     return (int)cudaGetLastError();
 }
 
-int launch_theta2(const Nl2Args& a, bool tmem, cudaStream_t st) {
-    const int nlines = a.b.nj * a.b.Nz;
-    if (tmem) {
-        using C = T2Cfg<true>;
-            if (int e = set_smem(k_theta2<true>, C::SMEM)) return e;
-        int grid = sm_count();
-        if (grid > (nlines + C::WARPS - 1) / C::WARPS) grid = (nlines + C::WARPS - 1) / C::WARPS;
-        k_theta2<true><<<grid, C::WARPS * 32, C::SMEM, st>>>(a);
-    } else {
-        using C = T2Cfg<false>;
-            if (int e = set_smem(k_theta2<false>, C::SMEM)) return e;
-        int grid = sm_count();
-        if (grid > (nlines + C::WARPS - 1) / C::WARPS) grid = (nlines + C::WARPS - 1) / C::WARPS;
-        k_theta2<false><<<grid, C::WARPS * 32, C::SMEM, st>>>(a);
-    }
+template <int NA, int NF> static int launch_theta2_t(const Nl2Args& a, cudaStream_t st) {
+    using C = T2Cfg<NA>;
+    const int nwarps = (a.b.nj * a.b.Nz + C::LPW - 1) / C::LPW;      // warps' worth of point-lines
+    if (int e = set_smem(k_theta2<NA, NF>, C::SMEM)) return e;
+    int grid = sm_count();
+    if (grid > (nwarps + T2_WARPS - 1) / T2_WARPS) grid = (nwarps + T2_WARPS - 1) / T2_WARPS;
+    k_theta2<NA, NF><<<grid, T2_WARPS * 32, C::SMEM, st>>>(a);
     return (int)cudaGetLastError();
+}
+
+int launch_zinv2(int na, const Nl2Args& a, cudaStream_t st) {
+    return na == 24 ? launch_zinv2_t<24>(a, st) : launch_zinv2_t<12>(a, st);
+}
+
+int launch_zfwd2(int na, const Nl2Args& a, cudaStream_t st) {
+    return na == 24 ? launch_zfwd2_t<24>(a, st) : launch_zfwd2_t<12>(a, st);
+}
+
+int launch_theta2(int na, const Nl2Args& a, cudaStream_t st) {
+    if (na == 24) return a.b.nf == 3 ? launch_theta2_t<24, 3>(a, st) : launch_theta2_t<24, 4>(a, st);
+    return a.b.nf == 3 ? launch_theta2_t<12, 3>(a, st) : launch_theta2_t<12, 4>(a, st);
 }
 
 }  // namespace nsc

@@ -1,24 +1,25 @@
-// nonlinear_v2.cuh -- transform kernels of the nonlinear term specialised for line length 768
-// (BASELINE.json configs[3], the headline workload: 3/2-padded 768 x 768 grid per radial node).
-// Same steps N1-N6 and the same intermediate layout as nonlinear_kernels.cuh; what changes:
+// nonlinear_v2.cuh -- transform kernels of the nonlinear term for the long line lengths 768 = 24 x 32 and
+// 384 = 12 x 32 (BASELINE.json configs[3]: 3/2-padded 768 x 768 grid per radial node, the headline workload;
+// configs[2]: 384 x 384, heated).  Same steps N1-N6 and the same intermediate layout as nonlinear_kernels.cuh;
+// what changes:
 //
-//   * the two-pass 24 x 32 transform of fft768.cuh: one shared-memory exchange per line instead of
-//     two, conflict-free, one warp per line and only warp-level barriers inside a transform;
+//   * the two-pass NA x 32 transform of fft_warp.cuh: one shared-memory exchange per line instead of two,
+//     conflict-free, one warp per 768-line (or per two 384-lines) and only warp-level barriers inside a transform;
 //   * k_dr     the radial derivative D1 f (N1) is taken once per evaluation by a marching kernel
 //              (one thread per (m, k) column, nine levels in registers), so that no transform
 //              kernel re-reads nine radial neighbours per line;
-//   * k_zinv2  four adjacent m-lines per CTA; the transposed [z][m] stores go through a swizzled
-//              shared-memory tile and leave as full 64-byte segments;
-//   * k_theta2 one (j, z) point-line per warp, the 12 real physical-space lines exist only in
-//              registers; the three velocity lines and one parked line live in a lane-private
-//              scratch -- Tensor Memory (tcgen05.st / tcgen05.ld, 256 columns per warp: TMEM as
-//              a 256 KB lane-private register spill space next to the 64 K registers) or shared
-//              memory (fallback variant);
-//   * k_zfwd2  cp.async double-buffered [z][4 m] tiles, forward transform, truncation, scaling,
+//   * k_zinv2  4 (8) adjacent m-lines per CTA; the transposed [z][m] stores go through a swizzled
+//              shared-memory tile and leave as full 64-byte (128-byte) segments;
+//   * k_theta2 one (j, z) point-line (two for length 384) per warp, the 12 (15 with temperature) real
+//              physical-space lines exist only in registers; the three velocity lines and one parked line live
+//              in a lane-private scratch in Tensor Memory (tcgen05.st / tcgen05.ld, 256 columns per warp: TMEM
+//              as a 256 KB lane-private register spill space next to the 64 K registers); optionally the
+//              per-level maxima of |u_r|, |u_theta|, |u_z| for the CFL rate of the step-size controller;
+//   * k_zfwd2  cp.async double-buffered [z][4 m] ([z][8 m]) tiles, forward transform, truncation, scaling,
 //              buoyancy.
 #pragma once
 #include <cstdint>
-#include "fft768.cuh"
+#include "fft_warp.cuh"
 #include "nonlinear_v2_args.h"
 
 namespace nsc {
@@ -101,52 +102,27 @@ __global__ void __launch_bounds__(DR_TB) k_dr(DrArgs a) {
     asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
-// ------------------------------------------------------------------------------------------
-
-// swizzled position (in 16-byte chunks) of (z, m_local) in a [768][4] tile: conflict free both for
-// lanes walking z (transform side) and for lanes walking (z, m_local) row-major (global side)
-__device__ __forceinline__ int tile4(int z, int ml) { return z * 4 + (ml ^ ((z >> 1) & 3)); }
-
-// axial mode index kk = k + K of padded-line index i (i <= K or i >= 768 - K), and k as a double
-struct ZBin {
-    int kk;
-    double kd;
-    bool ok;
-};
-__device__ __forceinline__ ZBin z_bin(int i, int K) {
-    ZBin b;
-    if (i <= K) {
-        b.kk = i + K;
-        b.kd = (double)i;
-        b.ok = true;
-    } else if (i >= f768::N - K) {
-        b.kk = i - f768::N + K;
-        b.kd = (double)(i - f768::N);
-        b.ok = true;
-    } else {
-        b.kk = 0;
-        b.kd = 0.0;
-        b.ok = false;
-    }
-    return b;
-}
-
-// S-layout slots that can hold non-zero spectral data when the mode count is <= 256 = 768 / 3:
-// t = 0..8 (bins 0..287) and t = 16..23 (bins 512..767); t = 9..15 is always zero padding.
-#define NSC_S_SLOTS(OP) OP(0) OP(1) OP(2) OP(3) OP(4) OP(5) OP(6) OP(7) OP(8) OP(16) OP(17) OP(18) OP(19) OP(20) OP(21) OP(22) OP(23)
-
+// ------------------------------------------------------------------------------------------ z kernels
 constexpr int Z2_WARPS = 4;
 constexpr int Z2_THREADS = Z2_WARPS * 32;
-constexpr size_t Z2_SMEM_X = sizeof(cd) * (size_t)(f768::XBUF * (1 + Z2_WARPS));
-constexpr size_t Z2_TILE = (size_t)f768::N * Z2_WARPS;                 // complex elements of one tile
-constexpr size_t Z2_SMEM_FWD = Z2_SMEM_X + sizeof(cd) * Z2_TILE;     // + the second tile buffer
 
-// ------------------------------------------------------------------------------------------ k_zinv2
-// work item = (field, level, tile of 4 adjacent m); three inverse transforms per line:
-// q = 1 (i kappa f), q = 0 (f), q = 2 (D1 f).  Each warp stages its spectral line in a private
-// shared-memory buffer filled by cp.async one transform ahead (f for two transforms, then D1 f,
-// then the next item's f), so no line waits in registers; the three transforms share one copy of
-// the code (instruction cache).
+template <int NA> struct Z2Cfg {
+    using G = fw::WGeo<NA>;
+    static constexpr int LPW = G::LPW;                           // spectral lines per warp
+    static constexpr int MT = Z2_WARPS * LPW;                    // m-lines per work item: 4 (768) or 8 (384)
+    static constexpr int LINE = (2 * G::NMAX + 1 + 7) / 8 * 8;   // staged spectral line (>= 2 K + 1): 520 / 264
+    static constexpr int TILE = G::N * MT;                       // complex elements of the [N][MT] tile (3072)
+    static constexpr int NIT = TILE / Z2_THREADS;                // tile elements per thread (24)
+    static constexpr size_t SMEM_INV = sizeof(cd) * (size_t)(fw::XBUF * (1 + Z2_WARPS) + LINE * LPW * Z2_WARPS);
+    static constexpr size_t SMEM_FWD = sizeof(cd) * (size_t)(fw::XBUF * (1 + Z2_WARPS) + TILE);
+    static_assert(TILE <= fw::XBUF * Z2_WARPS, "the tile overlays the exchange matrices");
+};
+
+// swizzle of the m_local index of row z of a [N][MT] tile: positions (in 16-byte chunks) z MT + (ml ^ swz(z)) are
+// conflict free both for lanes walking z (transform side) and for lanes walking (z, m_local) row-major (global side)
+template <int MT> __device__ __forceinline__ int swz(int z) { return MT == 4 ? ((z >> 1) & 3) : (z & 7); }
+template <int MT> __device__ __forceinline__ int tile_pos(int z, int ml) { return z * MT + (ml ^ swz<MT>(z)); }
+
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
@@ -155,33 +131,43 @@ __device__ __forceinline__ void cp_async_commit_wait_all() {
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
 }
 
-constexpr int Z2_LINE = 520;      // complex elements of a staged spectral line (>= 2 K + 1 = 513)
-constexpr size_t Z2_SMEM_INV = sizeof(cd) * (size_t)(f768::XBUF * (1 + Z2_WARPS) + Z2_LINE * Z2_WARPS);
-
+// ------------------------------------------------------------------------------------------ k_zinv2
+// work item = (field, level, tile of MT adjacent m); two or three inverse transforms per line:
+// q = 1 (i kappa f), q = 0 (f), [q = 2 (D1 f)].  Each warp stages its spectral line(s) in a private
+// shared-memory buffer filled by cp.async one transform ahead (f for two transforms, then D1 f,
+// then the next item's f), so no line waits in registers; the transforms share one copy of
+// the code (instruction cache).
+template <int NA>
 __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
-    using namespace f768;
+    using namespace fw;
+    using G = WGeo<NA>;
+    using C = Z2Cfg<NA>;
+    constexpr int N = G::N, LPW = C::LPW, MT = C::MT;
     const NlArgs& a = A.b;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cd* tw = reinterpret_cast<cd*>(smem_raw);
-    cd* tile = tw + XBUF;                               // [768][4] tile, overlays the 4 matrices
+    cd* tile = tw + XBUF;                               // [N][MT] tile, overlays the 4 matrices
     const int warp = threadIdx.x >> 5, tau = threadIdx.x & 31;
     cd* buf = tile + warp * XBUF;
-    cd* line = tw + XBUF * (1 + Z2_WARPS) + warp * Z2_LINE;
-    load_twiddles(tw, A.tw768);
-    const int mtiles = a.MP / 4;
+    cd* line = tw + XBUF * (1 + Z2_WARPS) + warp * (LPW * C::LINE);
+    load_twiddles(tw, A.tw_z);
+    const int mtiles = a.MP / MT;
     const size_t plane = (size_t)a.M1 * a.NK;
     const size_t qstride = (size_t)N * a.MP;
     const double taud = (double)tau;
     const int NKc = a.NK;
 
-    // requests this warp's spectral line of item `it` from `base` (a field or its radial derivative)
+    // requests this warp's spectral line(s) of item `it` from `base` (a field or its radial derivative)
     auto fetch = [&](const cd* base, int it) {
         const int mt = it % mtiles, r = it / mtiles;
         const int jl = r % a.nj;
-        const int m = mt * 4 + warp;
-        if (m < a.M1) {
-            const cd* src = base + (size_t)(a.j0 + jl) * plane + (size_t)m * NKc;
-            for (int i = tau; i < NKc; i += 32) cp_async16(line + i, src + i);
+#pragma unroll
+        for (int l = 0; l < LPW; ++l) {
+            const int m = mt * MT + warp * LPW + l;
+            if (m < a.M1) {
+                const cd* src = base + (size_t)(a.j0 + jl) * plane + (size_t)m * NKc;
+                for (int i = tau; i < NKc; i += 32) cp_async16(line + l * C::LINE + i, src + i);
+            }
         }
     };
     auto field_of = [&](int it) { return (it / mtiles) / a.nj; };
@@ -195,7 +181,6 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
     for (; item < A.nitems; item += gridDim.x) {
         const int mt = item % mtiles, r = item / mtiles;
         const int jl = r % a.nj, fi = r / a.nj;
-        const bool vm = (mt * 4 + warp) < a.M1;
 #pragma unroll 1
         for (int s = 0; s < ns; ++s) {
             const int q = (s == 0) ? 1 : (s == 1 ? 0 : 2);
@@ -205,22 +190,24 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
                 __syncwarp();
             }
             const double mult = (s == 0) ? A.alpha : 0.0;
-            {
-#define NSC_SET(T)                                                                              \
-    {                                                                                           \
-        const int kk = (T <= 8) ? tau + 32 * T + a.K : tau + 32 * T - N + a.K;                  \
-        const bool ok = vm && ((T <= 8) ? (tau + 32 * T <= a.K) : (tau + 32 * T >= N - a.K));   \
-        cd v = ok ? line[kk] : mk(0.0, 0.0);                                                    \
-        if (s == 0) {                                                                           \
-            const double kd = (T <= 8) ? taud + (double)(32 * T) : taud + (double)(32 * T - N); \
-            v = (mult * kd) * mul_i(v);                                                         \
-        }                                                                                       \
-        x[T] = v;                                                                               \
-    }
-                NSC_S_SLOTS(NSC_SET)
-#undef NSC_SET
 #pragma unroll
-                for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
+            for (int t = 0; t < NV; ++t) {
+                const int l = t / NA, tt = t % NA;
+                if (!G::slot_live(tt)) {
+                    x[t] = mk(0.0, 0.0);
+                    continue;
+                }
+                const bool pos = G::slot_pos(tt);
+                const int bin = tau + 32 * tt;
+                const bool vm = (mt * MT + warp * LPW + l) < a.M1;
+                const bool ok = vm && (pos ? (bin <= a.K) : (bin >= N - a.K));
+                const int kk = pos ? bin + a.K : bin - N + a.K;
+                cd v = ok ? line[l * C::LINE + kk] : mk(0.0, 0.0);
+                if (s == 0) {
+                    const double kd = pos ? taud + (double)(32 * tt) : taud + (double)(32 * tt - N);
+                    v = (mult * kd) * mul_i(v);
+                }
+                x[t] = v;
             }
             if (s >= 1) {                               // the staged line is consumed: request the next one
                 __syncwarp();
@@ -231,27 +218,27 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
                     if (nxt < A.nitems) fetch(a.f[field_of(nxt)], nxt);
                 }
             }
-            s2p<+1>(x, buf, tw, tau);
-            // P-layout result of this warp's line -> tile -> [z][m] work array in 64-byte segments
+            s2p<NA, +1>(x, buf, tw, tau);
+            // P-layout result of this warp's line(s) -> tile -> [z][m] work array in MT * 16-byte segments
             __syncthreads();                            // all warps left their exchange matrices
-            if (tau < NA) {
+            if (tau < NV) {
+                const int ml = warp * LPW + tau / NA;
 #pragma unroll
-                for (int e = 0; e < 32; ++e) tile[tile4(p_idx(e, tau), warp)] = x[e];
+                for (int e = 0; e < 32; ++e) tile[tile_pos<MT>(G::p_idx(e, tau), ml)] = x[e];
             }
             __syncthreads();
-            cd* dst = a.zbuf + ((size_t)jl * 3 * a.nf + (3 * fi + q)) * qstride + mt * 4;
+            cd* dst = a.zbuf + ((size_t)jl * 3 * a.nf + (3 * fi + q)) * qstride + mt * MT;
             // all shared-memory reads first, then all stores (the transform's registers are free here): no
             // store has to release its source registers before the next read can issue
             {
-                constexpr int NIT = (N * 4) / Z2_THREADS;       // 24
-                cd v[NIT];
+                cd v[C::NIT];
 #pragma unroll
-                for (int it = 0; it < NIT; ++it) v[it] = tile[threadIdx.x + it * Z2_THREADS];
-                // id = threadIdx.x + 128 it: z = id >> 2 = (threadIdx.x >> 2) + 32 it, c = id & 3 = threadIdx.x & 3
-                const int z0 = threadIdx.x >> 2, c0 = threadIdx.x & 3;
-                cd* d0 = dst + (size_t)z0 * a.MP + (c0 ^ ((z0 >> 1) & 3));  // (z >> 1) & 3 is the same for z0 + 32 it
+                for (int it = 0; it < C::NIT; ++it) v[it] = tile[threadIdx.x + it * Z2_THREADS];
+                // id = threadIdx.x + 128 it: z = id / MT = z0 + (128 / MT) it, c = id % MT = c0; swz(z) = swz(z0)
+                const int z0 = threadIdx.x / MT, c0 = threadIdx.x % MT;
+                cd* d0 = dst + (size_t)z0 * a.MP + (c0 ^ swz<MT>(z0));
 #pragma unroll
-                for (int it = 0; it < NIT; ++it) d0[(size_t)(32 * it) * a.MP] = v[it];
+                for (int it = 0; it < C::NIT; ++it) d0[(size_t)((Z2_THREADS / MT) * it) * a.MP] = v[it];
             }
             __syncthreads();                            // tile free again
         }
@@ -260,31 +247,34 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
 }
 
 // ------------------------------------------------------------------------------------------ k_zfwd2
-// work item = (field, level, tile of 4 adjacent m).  The [768][4] tile of theta-transformed
-// products arrives by cp.async (64-byte segments) while the previous item is being transformed.
-
+// work item = (field, level, tile of MT adjacent m).  The [N][MT] tile of theta-transformed
+// products arrives by cp.async (MT * 16-byte segments) while the previous item is being transformed.
+template <int NA>
 __global__ void __launch_bounds__(Z2_THREADS, 2) k_zfwd2(Nl2Args A) {
-    using namespace f768;
+    using namespace fw;
+    using G = WGeo<NA>;
+    using C = Z2Cfg<NA>;
+    constexpr int N = G::N, LPW = C::LPW, MT = C::MT;
     const NlArgs& a = A.b;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cd* tw = reinterpret_cast<cd*>(smem_raw);
     const int warp = threadIdx.x >> 5, tau = threadIdx.x & 31;
     cd* buf = tw + XBUF + warp * XBUF;
     cd* tile = tw + XBUF * (1 + Z2_WARPS);
-    load_twiddles(tw, A.tw768);
-    const int a23 = tau < NA ? tau : NA - 1;
-    const int mtiles = a.MP / 4;
+    load_twiddles(tw, A.tw_z);
+    const int a23 = tau < NV ? tau : NV - 1;
+    const int mtiles = a.MP / MT;
     const size_t qstride = (size_t)N * a.MP;
 
     auto fetch = [&](int it) {
         const int mt = it % mtiles, r = it / mtiles;
         const int jl = r % a.nj, fi = r / a.nj;
-        const cd* src = a.tbuf + ((size_t)jl * a.nf + fi) * qstride + mt * 4;
+        const cd* src = a.tbuf + ((size_t)jl * a.nf + fi) * qstride + mt * MT;
 #pragma unroll 4
-        for (int k = 0; k < (N * 4) / Z2_THREADS; ++k) {
+        for (int k = 0; k < C::NIT; ++k) {
             const int id = threadIdx.x + k * Z2_THREADS;
-            const int z = id >> 2, c = id & 3;
-            cp_async16(tile + id, src + (size_t)z * a.MP + (c ^ ((z >> 1) & 3)));
+            const int z = id / MT, c = id % MT;
+            cp_async16(tile + id, src + (size_t)z * a.MP + (c ^ swz<MT>(z)));
         }
     };
     int item = blockIdx.x;
@@ -292,49 +282,51 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zfwd2(Nl2Args A) {
     for (; item < A.nitems; item += gridDim.x) {
         const int mt = item % mtiles, r = item / mtiles;
         const int jl = r % a.nj, fi = r / a.nj;
-        const int j = a.j0 + jl, m = mt * 4 + warp;
+        const int j = a.j0 + jl;
         cp_async_commit_wait_all();
         __syncthreads();                                 // the tile (and, first time, tw) is complete
         cd x[32];
+        {
+            const int ml = warp * LPW + a23 / NA;
 #pragma unroll
-        for (int e = 0; e < 32; ++e) x[e] = tile[tile4(p_idx(e, a23), warp)];
-        __syncthreads();                                 // every warp holds its line: the tile is free
+            for (int e = 0; e < 32; ++e) x[e] = tile[tile_pos<MT>(G::p_idx(e, a23), ml)];
+        }
+        __syncthreads();                                 // every warp holds its line(s): the tile is free
         if (item + (int)gridDim.x < A.nitems) fetch(item + gridDim.x);
-        p2s<-1>(x, buf, tw, tau);
-        if (m < a.M1) {
-            const size_t off = ((size_t)j * a.M1 + m) * a.NK;
-            cd* dst = a.out[fi] + off;
-            const bool add_buoy = (fi == 2) && (a.buoy != 0.0);
-            const cd* Th = a.f[add_buoy ? 3 : 0] + off;
-#define NSC_ST(T)                                          \
-    {                                                      \
-        ZBin zb = z_bin(tau + 32 * T, a.K);                \
-        if (zb.ok) {                                       \
-            cd v = a.scale * x[T];                         \
-            if (add_buoy) {                                \
-                cd th = Th[zb.kk];                         \
-                v.x = fma(a.buoy, th.x, v.x);              \
-                v.y = fma(a.buoy, th.y, v.y);              \
-            }                                              \
-            dst[zb.kk] = v;                                \
-        }                                                  \
-    }
-            NSC_S_SLOTS(NSC_ST)
-#undef NSC_ST
+        p2s<NA, -1>(x, buf, tw, tau);
+        const bool add_buoy = (fi == 2) && (a.buoy != 0.0);
+#pragma unroll
+        for (int t = 0; t < NV; ++t) {
+            const int l = t / NA, tt = t % NA;
+            if (!G::slot_live(tt)) continue;
+            const int m = mt * MT + warp * LPW + l;
+            const bool pos = G::slot_pos(tt);
+            const int bin = tau + 32 * tt;
+            const bool ok = (m < a.M1) && (pos ? (bin <= a.K) : (bin >= N - a.K));
+            if (ok) {
+                const int kk = pos ? bin + a.K : bin - N + a.K;
+                const size_t off = ((size_t)j * a.M1 + m) * a.NK + kk;
+                cd v = a.scale * x[t];
+                if (add_buoy) {
+                    const cd th = a.f[3][off];
+                    v.x = fma(a.buoy, th.x, v.x);
+                    v.y = fma(a.buoy, th.y, v.y);
+                }
+                a.out[fi][off] = v;
+            }
         }
     }
     cp_async_commit_wait_all();
 }
 
 // ------------------------------------------------------------------------------------------ scratch
-// Lane-private scratch of k_theta2: NSLOT lines of 32 doubles per lane.  Two implementations with
-// the same interface: st(slot, v[32]) / ld(slot, v[32]), both warp-collective.
+// Lane-private scratch of k_theta2: T2_NSLOT lines of 32 doubles per lane in Tensor Memory.  A CTA of 8 warps owns
+// all 512 columns of its SM's TMEM; warp w may touch the 32 lanes of its quadrant (w & 3) only, so warps w and
+// w + 4 share lanes and split the columns: 256 columns = 128 doubles per thread = 4 slots of 32.  tcgen05.st / .ld
+// with shape 32x32b move one 32-bit column per register per lane; x16 = 8 doubles per instruction.
 constexpr int T2_NSLOT = 4;            // U_r, U_theta / r, U_z, one parked line
+constexpr int T2_WARPS = 8;
 
-// (1) Tensor Memory.  A CTA of 8 warps owns all 512 columns of its SM's TMEM; warp w may touch the
-// 32 lanes of its quadrant (w & 3) only, so warps w and w + 4 share lanes and split the columns:
-// 256 columns = 128 doubles per thread = 4 slots of 32.  tcgen05.st / .ld with shape 32x32b move one
-// 32-bit column per register per lane; x16 = 8 doubles per instruction.
 struct TmemScratch {
     uint32_t base;        // TMEM address (lane << 16 | column) of this warp's slot 0
     __device__ __forceinline__ void st8(uint32_t addr, const double* v) const {
@@ -359,318 +351,195 @@ struct TmemScratch {
             : "r"(addr)
             : "memory");
     }
-    __device__ __forceinline__ void ld8(uint32_t addr, double* v) const {
-        uint32_t r[16];
-        ld8_raw(addr, r);
-        wait_ld();
-#pragma unroll
-        for (int i = 0; i < 8; ++i) v[i] = __hiloint2double((int)r[2 * i + 1], (int)r[2 * i]);
-    }
-    // the registers of every ld8 issued so far are valid after this
+    // the registers of every ld8_raw issued so far are valid after this
     __device__ __forceinline__ void wait_ld() const { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-    __device__ __forceinline__ void st(int slot, const double* v) const {
-#pragma unroll
-        for (int c = 0; c < 4; ++c) st8(base + slot * 64 + c * 16, v + 8 * c);
-        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-    }
-    __device__ __forceinline__ void ld(int slot, double* v) const {
-#pragma unroll
-        for (int c = 0; c < 4; ++c) ld8(base + slot * 64 + c * 16, v + 8 * c);
-    }
 };
 
-// (2) shared memory: [slot][e][24 lanes] doubles per warp (lanes >= 24 hold nothing)
-struct SmemScratch {
-    double* base;         // this warp's block of T2_NSLOT * 32 * 24 doubles, already offset by the lane
-    bool active;
-    __device__ __forceinline__ void st(int slot, const double* v) const {
-        if (active)
-#pragma unroll
-            for (int e = 0; e < 32; ++e) base[(slot * 32 + e) * f768::NA] = v[e];
-    }
-    __device__ __forceinline__ void ld(int slot, double* v) const {
-#pragma unroll
-        for (int e = 0; e < 32; ++e) v[e] = base[(slot * 32 + e) * f768::NA];
-    }
+// chunked access (8 doubles = elements 8 c .. 8 c + 7 of a slot); split form: sc_ld8_raw (issue) ... sc_wait_ld
+// ... sc_unpack8 (use), so that several loads share one wait
+struct Raw8 {
+    uint32_t r[16];
 };
-
-template <bool TMEM> struct T2Cfg;
-constexpr int T2_STAGE = 264;      // complex elements of one staged half-spectral line (>= M + 1 = 257)
-template <> struct T2Cfg<true> {
-    static constexpr int WARPS = 8;
-    using Scratch = TmemScratch;
-    // twiddles + one exchange matrix and one staged line pair per warp; more than half of the SM's
-    // shared memory, so exactly one CTA (the owner of all 512 TMEM columns) is resident per SM
-    static constexpr size_t SMEM = sizeof(cd) * ((size_t)f768::XBUF * (1 + WARPS) + (size_t)2 * T2_STAGE * WARPS);
-};
-template <> struct T2Cfg<false> {
-    static constexpr int WARPS = 5;
-    using Scratch = SmemScratch;
-    static constexpr size_t SMEM = sizeof(cd) * ((size_t)f768::XBUF * (1 + WARPS) + (size_t)2 * T2_STAGE * WARPS) +
-                                   sizeof(double) * (size_t)WARPS * T2_NSLOT * 32 * f768::NA;
-};
-
-// chunked access (8 doubles = elements 8 c .. 8 c + 7 of a slot)
 __device__ __forceinline__ void sc_st8(const TmemScratch& s, int slot, int c, const double* v) {
     s.st8(s.base + slot * 64 + c * 16, v);
-}
-__device__ __forceinline__ void sc_ld8(const TmemScratch& s, int slot, int c, double* v) {
-    s.ld8(s.base + slot * 64 + c * 16, v);
 }
 __device__ __forceinline__ void sc_fence(const TmemScratch&) {
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
-__device__ __forceinline__ void sc_st8(const SmemScratch& s, int slot, int c, const double* v) {
-    if (s.active)
-#pragma unroll
-        for (int i = 0; i < 8; ++i) s.base[(slot * 32 + c * 8 + i) * f768::NA] = v[i];
-}
-__device__ __forceinline__ void sc_ld8(const SmemScratch& s, int slot, int c, double* v) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) v[i] = s.base[(slot * 32 + c * 8 + i) * f768::NA];
-}
-__device__ __forceinline__ void sc_fence(const SmemScratch&) {}
-// split form: sc_ld8_raw (issue) ... sc_wait_ld ... sc_unpack8 (use), so that several loads share one wait
-struct Raw8 {
-    uint32_t r[16];
-};
 __device__ __forceinline__ void sc_ld8_raw(const TmemScratch& s, int slot, int c, Raw8& q) {
     s.ld8_raw(s.base + slot * 64 + c * 16, q.r);
 }
-__device__ __forceinline__ void sc_ld8_raw(const SmemScratch& s, int slot, int c, Raw8& q) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const double v = s.base[(slot * 32 + c * 8 + i) * f768::NA];
-        q.r[2 * i] = (uint32_t)__double2loint(v);
-        q.r[2 * i + 1] = (uint32_t)__double2hiint(v);
-    }
-}
 __device__ __forceinline__ void sc_wait_ld(const TmemScratch& s) { s.wait_ld(); }
-__device__ __forceinline__ void sc_wait_ld(const SmemScratch&) {}
 __device__ __forceinline__ void sc_unpack8(const Raw8& q, double* v) {
 #pragma unroll
     for (int i = 0; i < 8; ++i) v[i] = __hiloint2double((int)q.r[2 * i + 1], (int)q.r[2 * i]);
 }
 
+template <int NA> struct T2Cfg {
+    using G = fw::WGeo<NA>;
+    static constexpr int LPW = G::LPW;                            // point-lines per warp
+    static constexpr int STAGE = (G::NMAX + 1 + 7) / 8 * 8;       // staged half-spectral line (>= M + 1): 264 / 136
+    // twiddles + one exchange matrix and one staged line pair per point-line per warp; more than half of the SM's
+    // shared memory, so exactly one CTA (the owner of all 512 TMEM columns) is resident per SM
+    static constexpr size_t SMEM = sizeof(cd) * ((size_t)fw::XBUF * (1 + T2_WARPS) + (size_t)2 * STAGE * LPW * T2_WARPS);
+};
+
 // ------------------------------------------------------------------------------------------ k_theta2
 // Z[i] = G_X(i) + i G_Y(i) in the S layout, G(m) = mult * line[m] (0 <= m <= M), G(-m) = conj G(m),
-// Im G(0) dropped (R6); mult = 1 or i n_m (d/dtheta, N1).  Slots t = 9..15 are zero padding.
-template <bool DX, bool DY, bool HAS_Y>
-__device__ __forceinline__ void load_pair768(cd* x, const cd* X, const cd* Y, int M, int tau, double taud,
-                                             double kth0) {
-#define NSC_POS(T)                                                    \
-    {                                                                 \
-        const int m = tau + 32 * T;                                   \
-        const bool ok = m <= M;                                       \
-        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
-        cd gy = (HAS_Y && ok) ? Y[m] : mk(0.0, 0.0);                  \
-        const double n = kth0 * (taud + (double)(32 * T));            \
-        if (DX) gx = n * mul_i(gx);                                   \
-        if (DY) gy = n * mul_i(gy);                                   \
-        if (T == 0 && tau == 0) {                                     \
-            gx.y = 0.0;                                               \
-            gy.y = 0.0;                                               \
-        }                                                             \
-        x[T] = mk(gx.x - gy.y, gx.y + gy.x);                          \
-    }
-#define NSC_NEG(T)                                                    \
-    {                                                                 \
-        const int m = f768::N - 32 * T - tau;                         \
-        const bool ok = m <= M;                                       \
-        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
-        cd gy = (HAS_Y && ok) ? Y[m] : mk(0.0, 0.0);                  \
-        const double n = kth0 * ((double)(f768::N - 32 * T) - taud);  \
-        if (DX) gx = n * mul_i(gx);                                   \
-        if (DY) gy = n * mul_i(gy);                                   \
-        x[T] = mk(gx.x + gy.y, gy.x - gx.y);                          \
-    }
-    NSC_POS(0) NSC_POS(1) NSC_POS(2) NSC_POS(3) NSC_POS(4) NSC_POS(5) NSC_POS(6) NSC_POS(7) NSC_POS(8)
-#pragma unroll
-    for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
-    NSC_NEG(16) NSC_NEG(17) NSC_NEG(18) NSC_NEG(19) NSC_NEG(20) NSC_NEG(21) NSC_NEG(22) NSC_NEG(23)
-#undef NSC_POS
-#undef NSC_NEG
-}
-
-// Splits the forward transform Z (S layout) of a packed real pair (a + i b) into the Hermitian half
-// lines A[m] = (Z[m] + conj Z[N-m]) / 2, B[m] = (Z[m] - conj Z[N-m]) / (2 i), m <= M (N5 truncation).
-// Z[N-m] of lane tau, slot T sits in lane (32 - tau) & 31, slot 23 - T (lane 0: its own slot 24 - T).
-template <bool HAS_B>
-__device__ __forceinline__ void store_pair768(const cd* x, cd* outA, cd* outB, int M, int tau) {
-    const int src = (32 - tau) & 31;
-#define NSC_OUT(T)                                                                 \
-    {                                                                              \
-        cd pz;                                                                     \
-        if (T == 8) {                                                              \
-            pz = x[16];                                                            \
-        } else {                                                                   \
-            pz.x = __shfl_sync(0xffffffffu, x[23 - T].x, src);                     \
-            pz.y = __shfl_sync(0xffffffffu, x[23 - T].y, src);                     \
-            if (tau == 0) pz = (T == 0) ? x[0] : x[(24 - T) % 24];                 \
-        }                                                                          \
-        const int m = tau + 32 * T;                                                \
-        if (m <= M) {                                                              \
-            const cd zm = conj(pz);                                                \
-            outA[m] = 0.5 * (x[T] + zm);                                           \
-            if (HAS_B) outB[m] = 0.5 * mul_mi(x[T] - zm);                          \
-        }                                                                          \
-    }
-    NSC_OUT(0) NSC_OUT(1) NSC_OUT(2) NSC_OUT(3) NSC_OUT(4) NSC_OUT(5) NSC_OUT(6) NSC_OUT(7) NSC_OUT(8)
-#undef NSC_OUT
-}
-
-__device__ __forceinline__ void store_pair768_rt(const cd* x, cd* outA, cd* outB, bool HAS_B, int M, int tau) {
-    const int src = (32 - tau) & 31;
-#define NSC_OUT(T)                                                                 \
-    {                                                                              \
-        cd pz;                                                                     \
-        if (T == 8) {                                                              \
-            pz = x[16];                                                            \
-        } else {                                                                   \
-            pz.x = __shfl_sync(0xffffffffu, x[23 - T].x, src);                     \
-            pz.y = __shfl_sync(0xffffffffu, x[23 - T].y, src);                     \
-            if (tau == 0) pz = (T == 0) ? x[0] : x[(24 - T) % 24];                 \
-        }                                                                          \
-        const int m = tau + 32 * T;                                                \
-        if (m <= M) {                                                              \
-            const cd zm = conj(pz);                                                \
-            outA[m] = 0.5 * (x[T] + zm);                                           \
-            if (HAS_B) outB[m] = 0.5 * mul_mi(x[T] - zm);                          \
-        }                                                                          \
-    }
-    NSC_OUT(0) NSC_OUT(1) NSC_OUT(2) NSC_OUT(3) NSC_OUT(4) NSC_OUT(5) NSC_OUT(6) NSC_OUT(7) NSC_OUT(8)
-#undef NSC_OUT
-}
-
-__device__ __forceinline__ void prefetch_l2(const void* p) {
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-}
-
-// run-time variant of load_pair768: one copy of the code serves all six inverse transforms of a
-// point-line, which keeps the kernel inside the instruction cache.  dx / dy select the d/dtheta
-// multiplier i n of the X / Y half; the four transforms without a derivative take the short branch
-// (uniform per warp), the other two blend (1, 0) / (0, n) multipliers arithmetically (no selects).
-__device__ __forceinline__ void load_pair768_rt(cd* x, const cd* X, const cd* Y, bool dx, bool dy, int M, int tau,
-                                                double taud, double kth0) {
+// Im G(0) dropped (R6); mult = 1 or i n_m (d/dtheta, N1).  Slots without a retained mode are zero padding.
+// One copy of the code serves all inverse transforms of a point-line, which keeps the kernel inside the instruction
+// cache.  dx / dy select the d/dtheta multiplier i n of the X / Y half; the transforms without a derivative take the
+// short branch (uniform per warp), the others blend (1, 0) / (0, n) multipliers arithmetically (no selects).
+// X, Y: the LPW staged lines of each half, STAGE apart.
+template <int NA>
+__device__ __forceinline__ void load_pair_rt(cd* x, const cd* X, const cd* Y, bool dx, bool dy, int M, int tau,
+                                             double taud, double kth0) {
+    using G = fw::WGeo<NA>;
+    constexpr int N = G::N, STAGE = T2Cfg<NA>::STAGE;
     if (!(dx || dy)) {
-#define NSC_POS(T)                                                    \
-    {                                                                 \
-        const int m = tau + 32 * T;                                   \
-        const bool ok = m <= M;                                       \
-        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
-        cd gy = ok ? Y[m] : mk(0.0, 0.0);                             \
-        if (T == 0 && tau == 0) {                                     \
-            gx.y = 0.0;                                               \
-            gy.y = 0.0;                                               \
-        }                                                             \
-        x[T] = mk(gx.x - gy.y, gx.y + gy.x);                          \
-    }
-#define NSC_NEG(T)                                                    \
-    {                                                                 \
-        const int m = f768::N - 32 * T - tau;                         \
-        const bool ok = m <= M;                                       \
-        const cd gx = ok ? X[m] : mk(0.0, 0.0);                       \
-        const cd gy = ok ? Y[m] : mk(0.0, 0.0);                       \
-        x[T] = mk(gx.x + gy.y, gy.x - gx.y);                          \
-    }
-        NSC_POS(0) NSC_POS(1) NSC_POS(2) NSC_POS(3) NSC_POS(4) NSC_POS(5) NSC_POS(6) NSC_POS(7) NSC_POS(8)
-        NSC_NEG(16) NSC_NEG(17) NSC_NEG(18) NSC_NEG(19) NSC_NEG(20) NSC_NEG(21) NSC_NEG(22) NSC_NEG(23)
-#undef NSC_POS
-#undef NSC_NEG
+#pragma unroll
+        for (int t = 0; t < fw::NV; ++t) {
+            const int l = t / NA, tt = t % NA;
+            if (!G::slot_live(tt)) {
+                x[t] = mk(0.0, 0.0);
+            } else if (G::slot_pos(tt)) {
+                const int m = tau + 32 * tt;
+                const bool ok = m <= M;
+                cd gx = ok ? X[l * STAGE + m] : mk(0.0, 0.0);
+                cd gy = ok ? Y[l * STAGE + m] : mk(0.0, 0.0);
+                if (tt == 0 && tau == 0) {
+                    gx.y = 0.0;
+                    gy.y = 0.0;
+                }
+                x[t] = mk(gx.x - gy.y, gx.y + gy.x);
+            } else {
+                const int m = N - 32 * tt - tau;
+                const bool ok = m <= M;
+                const cd gx = ok ? X[l * STAGE + m] : mk(0.0, 0.0);
+                const cd gy = ok ? Y[l * STAGE + m] : mk(0.0, 0.0);
+                x[t] = mk(gx.x + gy.y, gy.x - gx.y);
+            }
+        }
     } else {
         // g' = (a + i b n) g with (a, b) = (1, 0) plain or (0, 1) derivative
         const double ax = dx ? 0.0 : 1.0, bx = dx ? kth0 : 0.0;
         const double ay = dy ? 0.0 : 1.0, by = dy ? kth0 : 0.0;
-#define NSC_POS(T)                                                    \
-    {                                                                 \
-        const int m = tau + 32 * T;                                   \
-        const bool ok = m <= M;                                       \
-        cd gx = ok ? X[m] : mk(0.0, 0.0);                             \
-        cd gy = ok ? Y[m] : mk(0.0, 0.0);                             \
-        if (T == 0 && tau == 0) {                                     \
-            gx.y = 0.0;                                               \
-            gy.y = 0.0;                                               \
-        }                                                             \
-        const double mr = taud + (double)(32 * T);                    \
-        const double bxn = bx * mr, byn = by * mr;                    \
-        const cd hx = mk(fma(-bxn, gx.y, ax * gx.x), fma(bxn, gx.x, ax * gx.y)); \
-        const cd hy = mk(fma(-byn, gy.y, ay * gy.x), fma(byn, gy.x, ay * gy.y)); \
-        x[T] = mk(hx.x - hy.y, hx.y + hy.x);                          \
-    }
-#define NSC_NEG(T)                                                    \
-    {                                                                 \
-        const int m = f768::N - 32 * T - tau;                         \
-        const bool ok = m <= M;                                       \
-        const cd gx = ok ? X[m] : mk(0.0, 0.0);                       \
-        const cd gy = ok ? Y[m] : mk(0.0, 0.0);                       \
-        const double mr = (double)(f768::N - 32 * T) - taud;          \
-        const double bxn = bx * mr, byn = by * mr;                    \
-        const cd hx = mk(fma(-bxn, gx.y, ax * gx.x), fma(bxn, gx.x, ax * gx.y)); \
-        const cd hy = mk(fma(-byn, gy.y, ay * gy.x), fma(byn, gy.x, ay * gy.y)); \
-        x[T] = mk(hx.x + hy.y, hy.x - hx.y);                          \
-    }
-        NSC_POS(0) NSC_POS(1) NSC_POS(2) NSC_POS(3) NSC_POS(4) NSC_POS(5) NSC_POS(6) NSC_POS(7) NSC_POS(8)
-        NSC_NEG(16) NSC_NEG(17) NSC_NEG(18) NSC_NEG(19) NSC_NEG(20) NSC_NEG(21) NSC_NEG(22) NSC_NEG(23)
-#undef NSC_POS
-#undef NSC_NEG
-    }
 #pragma unroll
-    for (int t = 9; t < 16; ++t) x[t] = mk(0.0, 0.0);
+        for (int t = 0; t < fw::NV; ++t) {
+            const int l = t / NA, tt = t % NA;
+            if (!G::slot_live(tt)) {
+                x[t] = mk(0.0, 0.0);
+            } else if (G::slot_pos(tt)) {
+                const int m = tau + 32 * tt;
+                const bool ok = m <= M;
+                cd gx = ok ? X[l * STAGE + m] : mk(0.0, 0.0);
+                cd gy = ok ? Y[l * STAGE + m] : mk(0.0, 0.0);
+                if (tt == 0 && tau == 0) {
+                    gx.y = 0.0;
+                    gy.y = 0.0;
+                }
+                const double mr = taud + (double)(32 * tt);
+                const double bxn = bx * mr, byn = by * mr;
+                const cd hx = mk(fma(-bxn, gx.y, ax * gx.x), fma(bxn, gx.x, ax * gx.y));
+                const cd hy = mk(fma(-byn, gy.y, ay * gy.x), fma(byn, gy.x, ay * gy.y));
+                x[t] = mk(hx.x - hy.y, hx.y + hy.x);
+            } else {
+                const int m = N - 32 * tt - tau;
+                const bool ok = m <= M;
+                const cd gx = ok ? X[l * STAGE + m] : mk(0.0, 0.0);
+                const cd gy = ok ? Y[l * STAGE + m] : mk(0.0, 0.0);
+                const double mr = (double)(N - 32 * tt) - taud;
+                const double bxn = bx * mr, byn = by * mr;
+                const cd hx = mk(fma(-bxn, gx.y, ax * gx.x), fma(bxn, gx.x, ax * gx.y));
+                const cd hy = mk(fma(-byn, gy.y, ay * gy.x), fma(byn, gy.x, ay * gy.y));
+                x[t] = mk(hx.x + hy.y, hy.x - hx.y);
+            }
+        }
+    }
 }
 
-// The six inverse transforms of a point-line as a table: work array index q = 3 field + kind
-// (kind 0 f, 1 d_z f, 2 d_r f) of the X and Y halves of the packed pair, d/dtheta flags.
-//   t : 0 (u_r, u_th)  1 (u_z, dr u_r)  2 (dth u_r, dz u_r)  3 (dr u_th, dth u_th)  4 (dz u_th, dr u_z)  5 (dth u_z, dz u_z)
-__device__ __forceinline__ int t2_qx(int t) { return (0x645060 >> (4 * t)) & 15; }
-__device__ __forceinline__ int t2_qy(int t) { return (0x783123 >> (4 * t)) & 15; }
+// Splits the forward transform Z (S layout) of a packed real pair (a + i b) into the Hermitian half
+// lines A[m] = (Z[m] + conj Z[N-m]) / 2, B[m] = (Z[m] - conj Z[N-m]) / (2 i), m <= M (N5 truncation).
+// Z[N-m] of lane tau, slot tt sits in lane (32 - tau) & 31, slot NA - 1 - tt (lane 0: its own slot (NA - tt) % NA).
+// outA / outB: line l of the warp at outA + l * lstep.
+template <int NA>
+__device__ __forceinline__ void store_pair_rt(const cd* x, cd* outA, cd* outB, size_t lstep, bool has_b, int M, int tau) {
+    using G = fw::WGeo<NA>;
+    constexpr int TTMAX = G::NMAX / 32;                  // the last positive slot: only lane 0 (m = NMAX) can be kept
+    const int src = (32 - tau) & 31;
+#pragma unroll
+    for (int l = 0; l < G::LPW; ++l) {
+#pragma unroll
+        for (int tt = 0; tt <= TTMAX; ++tt) {
+            cd pz;
+            if (tt == TTMAX) {
+                pz = x[l * NA + NA - tt];
+            } else {
+                pz.x = __shfl_sync(0xffffffffu, x[l * NA + NA - 1 - tt].x, src);
+                pz.y = __shfl_sync(0xffffffffu, x[l * NA + NA - 1 - tt].y, src);
+                if (tau == 0) pz = x[l * NA + (NA - tt) % NA];
+            }
+            const int m = tau + 32 * tt;
+            if (m <= M) {
+                const cd zm = conj(pz);
+                outA[l * lstep + m] = 0.5 * (x[l * NA + tt] + zm);
+                if (has_b) outB[l * lstep + m] = 0.5 * mul_mi(x[l * NA + tt] - zm);
+            }
+        }
+    }
+}
 
-template <bool TMEM>
-__global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A) {
-    using namespace f768;
-    using Cfg = T2Cfg<TMEM>;
+// The inverse transforms of a point-line as a table: work array index q = 3 field + kind (kind 0 f, 1 d_z f,
+// 2 d_r f) of the X and Y halves of the packed pair; d/dtheta flags: X for t = 2, 5, Y for t = 3, 6.
+//   t : 0 (u_r, u_th)  1 (u_z, dr u_r)  2 (dth u_r, dz u_r)  3 (dr u_th, dth u_th)  4 (dz u_th, dr u_z)
+//       5 (dth u_z, dz u_z)  6 (dr T, dth T)  7 (dz T, -)      [6, 7 with temperature only]
+__device__ __forceinline__ int t2_qx(int t) { return (int)((0xAB645060u >> (4 * t)) & 15u); }
+__device__ __forceinline__ int t2_qy(int t) { return (int)((0xA9783123u >> (4 * t)) & 15u); }
+
+template <int NA, int NF>
+__global__ void __launch_bounds__(T2_WARPS * 32, 1) k_theta2(Nl2Args A) {
+    using namespace fw;
+    using G = WGeo<NA>;
+    using Cfg = T2Cfg<NA>;
+    constexpr int LPW = Cfg::LPW, STAGE = Cfg::STAGE;
+    constexpr int NT = NF == 3 ? 6 : 8;                  // inverse transforms per point-line
     const NlArgs& a = A.b;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t tmem_base_s;
     cd* tw = reinterpret_cast<cd*>(smem_raw);
     const int warp = threadIdx.x >> 5, tau = threadIdx.x & 31;
     cd* buf = tw + XBUF * (1 + warp);
-    const int a23 = tau < NA ? tau : NA - 1;
-    load_twiddles(tw, A.tw768);
-    typename Cfg::Scratch sc;
-    if constexpr (TMEM) {
-        if (warp == 0) {
-            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&tmem_base_s);
-            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(dst) : "memory");
-            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-        }
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        sc.base = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 256);
-    } else {
-        double* sb = reinterpret_cast<double*>(tw + XBUF * (1 + Cfg::WARPS) + 2 * T2_STAGE * Cfg::WARPS);
-        sc.base = sb + (size_t)warp * T2_NSLOT * 32 * NA + a23;
-        sc.active = tau < NA;
-        __syncthreads();
+    load_twiddles(tw, A.tw_t);
+    TmemScratch sc;
+    if (warp == 0) {
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&tmem_base_s);
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(dst) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    sc.base = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 256);
     const int M = a.M;
     const double taud = (double)tau, kth0 = A.ktheta0;
     const size_t qstride = (size_t)a.Nz * a.MP;
-    const int nlines = a.nj * a.Nz;
-    const int lstride = gridDim.x * Cfg::WARPS;
-    // this warp's staged line pair (X, Y) of the next inverse transform, filled by cp.async
-    cd* stX = tw + XBUF * (1 + Cfg::WARPS) + 2 * T2_STAGE * warp;
-    cd* stY = stX + T2_STAGE;
+    const int nlines = a.nj * a.Nz;                      // even; the LPW lines of a warp share their radial level
+    const int lstride = gridDim.x * T2_WARPS * LPW;
+    // this warp's staged line pairs (X then Y, LPW lines each) of the next inverse transform, filled by cp.async
+    cd* stX = tw + XBUF * (1 + T2_WARPS) + 2 * STAGE * LPW * warp;
+    cd* stY = stX + STAGE * LPW;
     auto stage = [&](int ln, int t) {
-        const size_t off = ((size_t)(ln / a.Nz) * 3 * a.nf * a.Nz + ln % a.Nz) * a.MP;
+        const size_t off = ((size_t)(ln / a.Nz) * 3 * a.nf * a.Nz + ln % a.Nz) * a.MP;     // line ln of q = 0; ln + 1: + MP
         const cd* X = a.zbuf + (size_t)t2_qx(t) * qstride + off;
         const cd* Y = a.zbuf + (size_t)t2_qy(t) * qstride + off;
-        for (int i = tau; i <= M; i += 32) {
-            cp_async16(stX + i, X + i);
-            cp_async16(stY + i, Y + i);
-        }
+#pragma unroll
+        for (int l = 0; l < LPW; ++l)
+            for (int i = tau; i <= M; i += 32) {
+                cp_async16(stX + l * STAGE + i, X + (size_t)l * a.MP + i);
+                cp_async16(stY + l * STAGE + i, Y + (size_t)l * a.MP + i);
+            }
     };
-    int line = blockIdx.x * Cfg::WARPS + warp;
+    int line = (blockIdx.x * T2_WARPS + warp) * LPW;
     if (line < nlines) stage(line, 0);
     for (; line < nlines; line += lstride) {
         const int jl = line / a.Nz;
@@ -680,19 +549,29 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
         cd x[32];
         double acc[32];
 #pragma unroll 1
-        for (int t = 0; t < 6; ++t) {
+        for (int t = 0; t < NT; ++t) {
             cp_async_commit_wait_all();
             __syncwarp();
-            load_pair768_rt(x, stX, stY, t == 2 || t == 5, t == 3, M, tau, taud, kth0);
+            load_pair_rt<NA>(x, stX, stY, t == 2 || t == 5, t == 3 || t == 6, M, tau, taud, kth0);
             __syncwarp();                                      // the staged pair is consumed: request the next one
-            if (t < 5)
+            if (t < NT - 1)
                 stage(line, t + 1);
             else if (line + lstride < nlines)
                 stage(line + lstride, 0);
-            s2p<+1>(x, buf, tw, tau);
+            s2p<NA, +1>(x, buf, tw, tau);
             sc_fence(sc);
             // physical-space stage (N4): slots 0 U_r, 1 U_theta / r, 2 U_z, 3 parked line
             if (t == 0) {
+                if (a.cfl) {                                   // per-level maxima for the CFL rate (step-size control)
+                    double m0 = 0.0, m1 = 0.0;
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) {
+                        m0 = fmax(m0, fabs(x[e].x));
+                        m1 = fmax(m1, fabs(x[e].y));
+                    }
+                    line_atomic_max<32>(a.cfl + 3 * (a.j0 + jl), m0, tau);
+                    line_atomic_max<32>(a.cfl + 3 * (a.j0 + jl) + 1, m1, tau);
+                }
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t1[8];
@@ -705,6 +584,12 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
                     sc_st8(sc, 1, c, t1);
                 }
             } else if (t == 1) {                               // acc = U_r d_r u_r
+                if (a.cfl) {
+                    double m2 = 0.0;
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) m2 = fmax(m2, fabs(x[e].x));
+                    line_atomic_max<32>(a.cfl + 3 * (a.j0 + jl) + 2, m2, tau);
+                }
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t2[8];
@@ -739,7 +624,7 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
                     }
                     sc_st8(sc, 3, c, t0);
                 }
-            } else if (t == 3) {                               // acc = U_r d_r u_th + (U_th / r) d_th u_th
+            } else if (t == 3 || t == 6) {                     // acc = U_r d_r f + (U_th / r) d_th f,  f = u_th or T
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t1[8];
@@ -779,7 +664,7 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
                     }
                     sc_st8(sc, 3, c, t2);
                 }
-            } else {                                           // N_z = -(u.grad u_z)  (buoyancy: k_zfwd)
+            } else if (t == 5) {                               // N_z = -(u.grad u_z)  (buoyancy: k_zfwd)
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     double t0[8], t1[8], t2[8];
@@ -797,24 +682,43 @@ __global__ void __launch_bounds__(T2Cfg<TMEM>::WARPS * 32, 1) k_theta2(Nl2Args A
                     for (int i = 0; i < 8; ++i) {
                         double s = fma(t1[i], x[8 * c + i].x, t0[i]);
                         s = fma(t2[i], x[8 * c + i].y, s);
-                        x[8 * c + i] = mk(-s, 0.0);
+                        if (NF == 3)
+                            x[8 * c + i] = mk(-s, 0.0);
+                        else
+                            t0[i] = -s;
+                    }
+                    if (NF == 4) sc_st8(sc, 3, c, t0);         // N_z parked until N_T is known
+                }
+            } else {                                           // t == 7: N_T = -(u.grad T); x <- (N_z, N_T)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double t2[8], t3[8];
+                    Raw8 q2;
+                    Raw8 q3;
+                    sc_ld8_raw(sc, 2, c, q2);
+                    sc_ld8_raw(sc, 3, c, q3);
+                    sc_wait_ld(sc);
+                    sc_unpack8(q2, t2);
+                    sc_unpack8(q3, t3);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const double s = fma(t2[i], x[8 * c + i].x, acc[8 * c + i]);
+                        x[8 * c + i] = mk(t3[i], -s);
                     }
                 }
             }
-            if (t >= 4) {                                      // N5: forward transform, truncation m <= M
-                p2s<-1>(x, buf, tw, tau);
+            if (t == 4 || t == NT - 1) {                       // N5: forward transform, truncation m <= M
+                p2s<NA, -1>(x, buf, tw, tau);
                 cd* O = a.tbuf + (size_t)(t == 4 ? 0 : 2) * qstride + loff;
-                store_pair768_rt(x, O, O + qstride, t == 4, M, tau);
+                store_pair_rt<NA>(x, O, O + qstride, (size_t)a.MP, t == 4 || NF == 4, M, tau);
             }
         }
     }
     cp_async_commit_wait_all();
-    if constexpr (TMEM) {
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();
-        if (warp == 0)
-            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base_s) : "memory");
-    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base_s) : "memory");
 }
 
 }  // namespace nsc

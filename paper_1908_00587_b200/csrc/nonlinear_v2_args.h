@@ -1,5 +1,5 @@
-// nonlinear_v2_args.h -- argument blocks and host-side launchers of the length-768 transform
-// kernels (nonlinear_v2.cuh), shared by the driver (nonlinear.cu) and the kernels' translation unit.
+// nonlinear_v2_args.h -- argument blocks and host-side launchers of the warp-transform kernels for the line
+// lengths 768 and 384 (nonlinear_v2.cuh), shared by the driver (nonlinear.cu) and the kernels' translation unit.
 #pragma once
 #include "nonlinear_kernels.cuh"
 
@@ -17,7 +17,8 @@ struct DrArgs {
 struct Nl2Args {
     NlArgs b;              // the generic argument block (fields, work arrays, sizes)
     const cd* dr[MAXF];    // radial derivatives of the input fields, spectral layout
-    const cd* tw768;       // [24][33] twiddle matrix of fft768.cuh
+    const cd* tw_z;        // [24][33] twiddle matrix of fft_warp.cuh for the z length (plan.cu)
+    const cd* tw_t;        // ... for the theta length
     double alpha;          // axial base wavenumber
     double ktheta0;        // azimuthal base wavenumber
     int nitems;            // work items of the launch
@@ -25,8 +26,11 @@ struct Nl2Args {
 
 // host-side launchers (nonlinear_v2.cu)
 int launch_dr(const DrArgs& a, int nf, cudaStream_t st);
-int launch_zinv2(const Nl2Args& a, cudaStream_t st);
-int launch_zfwd2(const Nl2Args& a, cudaStream_t st);
-int launch_theta2(const Nl2Args& a, bool tmem, cudaStream_t st);
+// na = 24 (length 768) or 12 (length 384); warp_na(n, modes): the na of length n if the warp kernels serve it
+int warp_na(int n, int modes);
+int warp_mtile(int na);    // m-lines per work item of the z kernels
+int launch_zinv2(int na, const Nl2Args& a, cudaStream_t st);
+int launch_zfwd2(int na, const Nl2Args& a, cudaStream_t st);
+int launch_theta2(int na, const Nl2Args& a, cudaStream_t st);
 
 }  // namespace nsc

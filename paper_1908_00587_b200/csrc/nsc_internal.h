@@ -43,7 +43,8 @@ struct Tables {               // all device pointers
     double* kap = nullptr;    // [2K+1]     kappa = k alpha
     cd* tw_t = nullptr;       // [N_theta]  exp(-2 pi i t / N_theta)
     cd* tw_z = nullptr;       // [N_z]
-    cd* tw768 = nullptr;      // [24][33]   exp(-2 pi i k1 n2 / 768) of fft768.cuh (if a length is 768)
+    cd* tw_wz = nullptr;      // [24][33]   twiddle matrix of fft_warp.cuh for N_z (if its length is 768 or 384)
+    cd* tw_wt = nullptr;      // [24][33]   ... for N_theta
 };
 
 }  // namespace nsc
@@ -74,9 +75,11 @@ struct nsc_ctx {
     nsc::cd* N1[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};
     nsc::cd* zbuf = nullptr;              // [JC][3 nf][N_z][MP]  z-transformed f, dz f, dr f
     nsc::cd* tbuf = nullptr;              // [JC][nf][N_z][MP]    theta-transformed products
-    nsc::cd* DR[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};       // D1 f (length-768 z pipeline)
-    bool z768 = false;                    // z transforms by k_dr + k_zinv2 / k_zfwd2
-    int t768 = 0;                         // theta transforms by k_theta2: 0 no, 1 shared-memory, 2 TMEM scratch
+    nsc::cd* DR[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};       // D1 f (warp z pipeline in several chunks)
+    int z_na = 0;                         // z transforms by k_dr + k_zinv2 / k_zfwd2 of fft_warp.cuh: 24 (768), 12 (384), 0 no
+    int t_na = 0;                         // theta transforms by k_theta2: 24, 12, 0 no
+    unsigned long long* cfl_max = nullptr;    // [N_r][3] per-level maxima of |u| (k_theta2 / k_theta), step-size control
+    bool want_cfl = false;                // the next launch_nonlinear accumulates them
     nsc::BandShape shH, shP;              // Helmholtz (9-wide rows) / Poisson (17-wide rows) envelopes
     nsc::BandFactors facH[4];             // u_+, u_-, u_z, T
     nsc::BandFactors facP;

@@ -11,7 +11,7 @@
 #include <cmath>
 #include <cstring>
 #include "nsc_internal.h"
-#include "fft768.cuh"
+#include "fft_warp.cuh"
 
 namespace nsc {
 
@@ -161,16 +161,19 @@ int build_plan(nsc_ctx* c) {
     if ((rc = upload(c, &c->t.kap, kap))) return rc;
     if ((rc = upload(c, &c->t.tw_t, twiddles(c->Nt)))) return rc;
     if ((rc = upload(c, &c->t.tw_z, twiddles(c->Nz)))) return rc;
-    if (c->Nt == f768::N || c->Nz == f768::N) {
-        // exp(-2 pi i k1 n2 / 768), k1 < 24, n2 < 32, row stride 33 (fft768.cuh)
-        std::vector<cd> t(f768::XBUF, mk(0.0, 0.0));
-        for (int k1 = 0; k1 < f768::NA; ++k1)
-            for (int n2 = 0; n2 < f768::NB; ++n2) {
-                ld a = 2 * pi_ld() * (ld)(k1 * n2) / f768::N;
-                t[k1 * f768::XS + n2] = mk((double)cosl(a), (double)(-sinl(a)));
+    // twiddle matrices of the warp transforms (fft_warp.cuh): tw[t][n2] = exp(-2 pi i (t % NA) n2 / N), row stride 33
+    auto warp_table = [&](int n, cd** dst) -> int {
+        const int na = n / fw::NB;
+        std::vector<cd> t(fw::XBUF, mk(0.0, 0.0));
+        for (int r = 0; r < fw::NV; ++r)
+            for (int n2 = 0; n2 < fw::NB; ++n2) {
+                ld a = 2 * pi_ld() * (ld)((r % na) * n2) / n;
+                t[r * fw::XS + n2] = mk((double)cosl(a), (double)(-sinl(a)));
             }
-        if ((rc = upload(c, &c->t.tw768, t))) return rc;
-    }
+        return upload(c, dst, t);
+    };
+    if (c->z_na && (rc = warp_table(c->Nz, &c->t.tw_wz))) return rc;
+    if (c->t_na && (rc = warp_table(c->Nt, &c->t.tw_wt))) return rc;
 
     // ---- band envelopes.  Helmholtz: identity rows at the walls (Dirichlet), stencil rows inside.
     c->shH.h_lo.resize(N);

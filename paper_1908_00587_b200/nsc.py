@@ -22,7 +22,7 @@ EXPORTS = (
     "nsc_set_state", "nsc_get_state", "nsc_set_state_host", "nsc_get_state_host",
     "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_step_iterated", "nsc_nusselt", "nsc_probe", "nsc_last_error", "nsc_device_bytes",
     "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name", "nsc_graph_replays",
-    "nsc_fp64_peak",
+    "nsc_fp64_peak", "nsc_cfl_rate", "nsc_advance", "nsc_mode_coefficient", "nsc_wave_speed",
 )
 NSC_NKERN = 11
 
@@ -44,6 +44,12 @@ class nsc_params(C.Structure):
         ("c", C.c_double), ("device", C.c_int), ("radial_chunk", C.c_int),
         ("linear_slices", C.c_int), ("no_graph", C.c_int),
     ]
+
+
+class nsc_advance_info(C.Structure):
+    _fields_ = [("t", C.c_double), ("dt_next", C.c_double), ("dt_last", C.c_double), ("dt_min", C.c_double),
+                ("dt_max", C.c_double), ("err_last", C.c_double), ("cfl_rate_last", C.c_double),
+                ("accepted", C.c_int), ("rejected", C.c_int), ("passes", C.c_int)]
 
 
 _lib = None
@@ -87,6 +93,10 @@ def load_library() -> C.CDLL:
     lib.nsc_graph_replays.argtypes = [vp]
     lib.nsc_graph_replays.restype = C.c_longlong
     lib.nsc_fp64_peak.argtypes = [i32, i32, C.POINTER(dbl)]
+    lib.nsc_cfl_rate.argtypes = [vp, C.POINTER(dbl)]
+    lib.nsc_advance.argtypes = [vp, dbl, i32, dbl, dbl, dbl, i32, C.POINTER(nsc_advance_info), C.POINTER(dbl)]
+    lib.nsc_mode_coefficient.argtypes = [vp, i32, i32, i32, i32, C.POINTER(dbl)]
+    lib.nsc_wave_speed.argtypes = [vp, i32, i32, i32, i32, dbl, i32, C.POINTER(dbl)]
     for name in EXPORTS:
         if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count", "nsc_kernel_name",
                         "nsc_graph_replays"):
@@ -217,6 +227,30 @@ class Context:
         k, err = C.c_int(0), C.c_double(0.0)
         self._check(self._lib.nsc_step_iterated(self._h, dt, tol, max_corr, C.byref(k), C.byref(err)))
         return k.value, err.value
+
+    def cfl_rate(self) -> float:
+        v = C.c_double(0.0)
+        self._check(self._lib.nsc_cfl_rate(self._h, C.byref(v)))
+        return v.value
+
+    def advance(self, t_end, max_steps, dt0, tol, cfl, max_corr):
+        """nsc_advance: returns (info dict, log) with log = list of (dt, passes, err, accepted) per attempt."""
+        info = nsc_advance_info()
+        log = (C.c_double * (4 * max_steps))()
+        self._check(self._lib.nsc_advance(self._h, t_end, max_steps, dt0, tol, cfl, max_corr, C.byref(info), log))
+        n = info.accepted + info.rejected
+        out = [(log[4 * i], int(log[4 * i + 1]), log[4 * i + 2], bool(log[4 * i + 3])) for i in range(n)]
+        return {f: getattr(info, f) for f, _ in nsc_advance_info._fields_}, out
+
+    def mode_coefficient(self, field, j, m, k) -> complex:
+        v = (C.c_double * 2)()
+        self._check(self._lib.nsc_mode_coefficient(self._h, field, j, m, k, v))
+        return complex(v[0], v[1])
+
+    def wave_speed(self, field, j, m, k, dt, n_steps) -> float:
+        v = C.c_double(0.0)
+        self._check(self._lib.nsc_wave_speed(self._h, field, j, m, k, dt, n_steps, C.byref(v)))
+        return v.value
 
     def step(self, dt):
         self._check(self._lib.nsc_step(self._h, float(dt)))

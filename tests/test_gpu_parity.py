@@ -539,3 +539,88 @@ def test_graph_replay_after_a_substep_with_another_dt(torch_cuda):
         if a is not None:
             assert np.isfinite(a).all()
             np.testing.assert_array_equal(a, b)
+
+
+@pytest.mark.parametrize("ci,N_r,M,K", [(0, 20, 4, 4), (2, 12, 16, 32), (1, 11, 64, 8), (3, 9, 256, 256), (2, 10, 128, 128)])
+def test_cfl_rate_matches_oracle(torch_cuda, ci, N_r, M, K):
+    """NEXT-1 (R17): nsc_cfl_rate (maxima of |u| per radial level gathered inside the theta kernels, generic and
+    warp-transform forms) against the oracle's cfl_rate on the physical grid."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    o = oracle_of(cfg, dft="fft")
+    with _ctx(cfg) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        st[0] = st[0] + 0.3 * st[1]                      # radial velocity of the size of the rotation: all three terms matter
+        ctx.set_state(*_dev(torch, st))
+        got = ctx.cfl_rate()
+        again = ctx.cfl_rate()
+    ref, _ = o.cfl_rate(st)
+    assert got == again
+    assert abs(got - ref) <= 1e-12 * ref
+
+
+@pytest.mark.parametrize("heated", [False, True])
+def test_step_size_controller_follows_the_oracle(torch_cuda, heated):
+    """NEXT-1 (R17): nsc_advance after an impulsive change of the rotation rate against the oracle's
+    advance: the same sequence of attempts (step sizes bit for bit, corrector passes, accept / reject), the same
+    corrector norms, the same state at t_end; rejected attempts leave the state untouched."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(2 if heated else 0, N_r=20, M=4, K=4)
+    if heated:
+        cfg = dict(cfg, Re_i=100.0, Re_o=0.0, Ra=2.0e3, dt=1e-3)
+    nf = nf_of(cfg)
+    cfg2 = dict(cfg, Re_i=400.0)
+    o1 = oracle_of(cfg, dft="fft")
+    st = synth.make_state(cfg, o1.r)
+    o2 = oracle_of(cfg2, dft="fft")
+    args = (8e-3, 200, 4e-3, 1e-7, 0.5, 2)
+    ref, t_ref, rlog = o2.advance(st, *args)
+    assert any(not ok for (_, _, _, ok) in rlog) and t_ref == args[0]
+    with _ctx(cfg2) as ctx:
+        ctx.set_state(*_dev(torch, st))
+        # one attempt only: rejected, nothing moves
+        info1, log1 = ctx.advance(args[0], 1, *args[2:])
+        assert info1["t"] == 0.0 and info1["rejected"] == 1 and info1["accepted"] == 0 and not log1[0][3]
+        for a, b in zip(ctx.state_to_host(), st):
+            if b is not None:
+                np.testing.assert_array_equal(a, b)
+        info, log = ctx.advance(*args)
+        got = ctx.state_to_host()
+    assert len(log) == len(rlog)
+    for (dt, k, err, ok), (rdt, rk, rerr, rok) in zip(log, rlog):
+        assert dt == rdt and k == rk and ok == rok
+        assert abs(err - rerr) <= 1e-4 * rerr + 1e-14
+    assert info["t"] == t_ref and info["accepted"] == sum(ok for (_, _, _, ok) in rlog)
+    assert info["rejected"] == len(rlog) - info["accepted"] and info["passes"] == sum(k for (_, k, _, _) in rlog)
+    assert info["dt_min"] == min(d for (d, _, _, ok) in rlog if ok) and info["dt_max"] == max(d for (d, _, _, ok) in rlog if ok)
+    check_parity(got[:nf], ref[:nf], TOL_STEP, cfg["K"], f"controller, {len(log)} attempts")
+
+
+def test_wave_speed_matches_oracle(torch_cuda):
+    """NEXT-3: nsc_wave_speed / nsc_mode_coefficient against the oracle's wave_speed on the pinned case (a
+    temperature disturbance carried by solid-body rotation, speed -> Omega) and on a velocity mode of cfg 1."""
+    torch = torch_cuda
+    Omega = 40.0
+    cfg = dict(synth.scaled_config(2, N_r=16, M=4, K=4), eta=0.5, Re_i=Omega * 1.0, Re_o=Omega * 2.0, Ra=1e-9, Pr=0.7)
+    o = oracle_of(cfg, dft="fft")
+    st = o.base_state_discrete()
+    x = o.r - o.r[0]
+    st[3][:, 2, 1 + o.p.K] += 1e-3 * x * (1 - x) * (1 + 0.5j)
+    ref, ref_state = o.wave_speed(st, 3, 7, 2, 1, 2.5e-4, 8)
+    with _ctx(cfg) as ctx:
+        ctx.set_state(*_dev(torch, st))
+        assert ctx.mode_coefficient(3, 7, 2, 1) == complex(st[3][7, 2, 1 + o.p.K])
+        got = ctx.wave_speed(3, 7, 2, 1, 2.5e-4, 8)
+        end = ctx.state_to_host()
+        with pytest.raises(Exception):
+            ctx.wave_speed(3, 7, 0, 1, 2.5e-4, 2)        # m = 0 has no azimuthal phase speed
+    assert abs(got - ref) <= 1e-9 * abs(ref) and abs(got - Omega) <= 3e-4 * Omega
+    check_parity(end[:4], ref_state[:4], TOL_STEP, cfg["K"], "state after the wave-speed steps")
+    cfg = synth.scaled_config(0, N_r=24, M=8, K=8)
+    o = oracle_of(cfg, dft="fft")
+    st = synth.make_state(cfg, o.r)
+    ref, _ = o.wave_speed(st, 1, 12, 1, 2, cfg["dt"], 5)
+    with _ctx(cfg) as ctx:
+        ctx.set_state(*_dev(torch, st))
+        got = ctx.wave_speed(1, 12, 1, 2, cfg["dt"], 5)
+    assert abs(got - ref) <= 1e-8 * abs(ref)
