@@ -52,14 +52,17 @@ template <int NA> static int launch_zfwd2_t(const Nl2Args& a, cudaStream_t st) {
     return (int)cudaGetLastError();
 }
 
-template <int NA, int NF> static int launch_theta2_t(const Nl2Args& a, cudaStream_t st) {
+template <int NA, int NF, bool CFL> static int launch_theta2_c(const Nl2Args& a, cudaStream_t st) {
     using C = T2Cfg<NA>;
     const int nwarps = (a.b.nj * a.b.Nz + C::LPW - 1) / C::LPW;      // warps' worth of point-lines
-    if (int e = set_smem(k_theta2<NA, NF>, C::SMEM)) return e;
+    if (int e = set_smem(k_theta2<NA, NF, CFL>, C::SMEM)) return e;
     int grid = sm_count();
     if (grid > (nwarps + T2_WARPS - 1) / T2_WARPS) grid = (nwarps + T2_WARPS - 1) / T2_WARPS;
-    k_theta2<NA, NF><<<grid, T2_WARPS * 32, C::SMEM, st>>>(a);
+    k_theta2<NA, NF, CFL><<<grid, T2_WARPS * 32, C::SMEM, st>>>(a);
     return (int)cudaGetLastError();
+}
+template <int NA, int NF> static int launch_theta2_t(const Nl2Args& a, cudaStream_t st) {
+    return a.b.cfl ? launch_theta2_c<NA, NF, true>(a, st) : launch_theta2_c<NA, NF, false>(a, st);
 }
 
 int launch_zinv2(int na, const Nl2Args& a, cudaStream_t st) {

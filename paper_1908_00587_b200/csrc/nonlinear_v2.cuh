@@ -189,23 +189,21 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zinv2(Nl2Args A) {
                 cp_async_commit_wait_all();
                 __syncwarp();
             }
-            const double mult = (s == 0) ? A.alpha : 0.0;
+            // v' = (am + i bm k) v: (am, bm) = (0, alpha) for d/dz = i kappa, (1, 0) otherwise (no branch per slot)
+            const double am = (s == 0) ? 0.0 : 1.0, bm = (s == 0) ? A.alpha : 0.0;
 #pragma unroll
             for (int t = 0; t < NV; ++t) {
                 const int l = t / NA, tt = t % NA;
-                if (!G::slot_live(tt)) {
-                    x[t] = mk(0.0, 0.0);
-                    continue;
-                }
-                const bool pos = G::slot_pos(tt);
-                const int bin = tau + 32 * tt;
-                const bool vm = (mt * MT + warp * LPW + l) < a.M1;
-                const bool ok = vm && (pos ? (bin <= a.K) : (bin >= N - a.K));
-                const int kk = pos ? bin + a.K : bin - N + a.K;
-                cd v = ok ? line[l * C::LINE + kk] : mk(0.0, 0.0);
-                if (s == 0) {
-                    const double kd = pos ? taud + (double)(32 * tt) : taud + (double)(32 * tt - N);
-                    v = (mult * kd) * mul_i(v);
+                cd v = mk(0.0, 0.0);
+                if (G::slot_live(tt)) {
+                    const bool pos = G::slot_pos(tt);
+                    const int bin = tau + 32 * tt;
+                    const bool vm = (mt * MT + warp * LPW + l) < a.M1;
+                    const bool ok = vm && (pos ? (bin <= a.K) : (bin >= N - a.K));
+                    const int kk = pos ? bin + a.K : bin - N + a.K;
+                    const cd g = ok ? line[l * C::LINE + kk] : mk(0.0, 0.0);
+                    const double kd = bm * (pos ? taud + (double)(32 * tt) : taud + (double)(32 * tt - N));
+                    v = mk(fma(-kd, g.y, am * g.x), fma(kd, g.x, am * g.y));
                 }
                 x[t] = v;
             }
@@ -296,23 +294,29 @@ __global__ void __launch_bounds__(Z2_THREADS, 2) k_zfwd2(Nl2Args A) {
         p2s<NA, -1>(x, buf, tw, tau);
         const bool add_buoy = (fi == 2) && (a.buoy != 0.0);
 #pragma unroll
-        for (int t = 0; t < NV; ++t) {
-            const int l = t / NA, tt = t % NA;
-            if (!G::slot_live(tt)) continue;
+        for (int l = 0; l < LPW; ++l) {
             const int m = mt * MT + warp * LPW + l;
-            const bool pos = G::slot_pos(tt);
-            const int bin = tau + 32 * tt;
-            const bool ok = (m < a.M1) && (pos ? (bin <= a.K) : (bin >= N - a.K));
-            if (ok) {
-                const int kk = pos ? bin + a.K : bin - N + a.K;
-                const size_t off = ((size_t)j * a.M1 + m) * a.NK + kk;
-                cd v = a.scale * x[t];
-                if (add_buoy) {
-                    const cd th = a.f[3][off];
-                    v.x = fma(a.buoy, th.x, v.x);
-                    v.y = fma(a.buoy, th.y, v.y);
+            if (m < a.M1) {
+                const size_t off = ((size_t)j * a.M1 + m) * a.NK;
+                cd* dst = a.out[fi] + off;
+                const cd* Th = a.f[add_buoy ? 3 : 0] + off;
+#pragma unroll
+                for (int tt = 0; tt < NA; ++tt) {
+                    if (G::slot_live(tt)) {
+                        const bool pos = G::slot_pos(tt);
+                        const int bin = tau + 32 * tt;
+                        if (pos ? (bin <= a.K) : (bin >= N - a.K)) {
+                            const int kk = pos ? bin + a.K : bin - N + a.K;
+                            cd v = a.scale * x[l * NA + tt];
+                            if (add_buoy) {
+                                const cd th = Th[kk];
+                                v.x = fma(a.buoy, th.x, v.x);
+                                v.y = fma(a.buoy, th.y, v.y);
+                            }
+                            dst[kk] = v;
+                        }
+                    }
                 }
-                a.out[fi][off] = v;
             }
         }
     }
@@ -496,7 +500,9 @@ __device__ __forceinline__ void store_pair_rt(const cd* x, cd* outA, cd* outB, s
 __device__ __forceinline__ int t2_qx(int t) { return (int)((0xAB645060u >> (4 * t)) & 15u); }
 __device__ __forceinline__ int t2_qy(int t) { return (int)((0xA9783123u >> (4 * t)) & 15u); }
 
-template <int NA, int NF>
+// CFL: also gather the per-level maxima of |u_r|, |u_theta|, |u_z| (a.cfl); an instantiation of its own, because
+// that code, even when skipped, lengthens the transform loop beyond the instruction cache (4 % slower).
+template <int NA, int NF, bool CFL>
 __global__ void __launch_bounds__(T2_WARPS * 32, 1) k_theta2(Nl2Args A) {
     using namespace fw;
     using G = WGeo<NA>;
@@ -562,7 +568,7 @@ __global__ void __launch_bounds__(T2_WARPS * 32, 1) k_theta2(Nl2Args A) {
             sc_fence(sc);
             // physical-space stage (N4): slots 0 U_r, 1 U_theta / r, 2 U_z, 3 parked line
             if (t == 0) {
-                if (a.cfl) {                                   // per-level maxima for the CFL rate (step-size control)
+                if constexpr (CFL) {                            // per-level maxima for the CFL rate (step-size control)
                     double m0 = 0.0, m1 = 0.0;
 #pragma unroll
                     for (int e = 0; e < 32; ++e) {
@@ -584,7 +590,7 @@ __global__ void __launch_bounds__(T2_WARPS * 32, 1) k_theta2(Nl2Args A) {
                     sc_st8(sc, 1, c, t1);
                 }
             } else if (t == 1) {                               // acc = U_r d_r u_r
-                if (a.cfl) {
+                if constexpr (CFL) {
                     double m2 = 0.0;
 #pragma unroll
                     for (int e = 0; e < 32; ++e) m2 = fmax(m2, fabs(x[e].x));
