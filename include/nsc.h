@@ -167,6 +167,18 @@ int nsc_mode_coefficient(nsc_ctx* ctx, int field, int j, int m, int k, double* h
  * The state advances by n_steps steps.  Synchronises the stream after every step. */
 int nsc_wave_speed(nsc_ctx* ctx, int field, int j, int m, int k, double dt, int n_steps, double* h_speed);
 
+/* Restart on another resolution ("At every restart, the spatial resolution can be
+ * changed using an automated interpolation and mode padding functionality"; reading R18): the state
+ * (u, T, p) of `src` is carried onto the radial grid and the mode set of `dst` and becomes the state of `dst`.
+ *   radial : degree-8 Lagrange interpolation on the nine source nodes around the source node nearest to each target
+ *            node (window start clamp(c - 4, 0, N_r,src - 9)); a target node that coincides with a source node takes
+ *            its value exactly;
+ *   modes  : coefficients of modes `src` does not hold are zero, modes `dst` does not hold are dropped.
+ * Both contexts must live on the same device and agree in eta, alpha and k_theta0 (NSC_EINVAL otherwise); N_r, M_theta,
+ * K_z, the grid family, Re_i, Re_o, Ra, Pr may differ.  A temperature field of `src` is dropped if `dst` has none;
+ * `dst` with temperature needs `src` with temperature.  `src` is unchanged.  Synchronises both streams. */
+int nsc_regrid(nsc_ctx* dst, nsc_ctx* src);
+
 /* Wall diagnostics of the current state (Fig. 3a): transfer at a wall
  * normalised by that of the basic state at the same parameters, from the mean mode (0,0):
  *   h_out[0], h_out[1]  heat-flux Nusselt number at the inner / outer wall, d_r T r ln(eta)  (nan if Ra = 0)

@@ -664,6 +664,47 @@ class Oracle:
                 dt_cur = self.dt_grid_floor(dt / 2)
         return state, t, log
 
+    # ---------------------------------------------------------------- NEXT-4: restart on another resolution
+    def regrid_matrix(self, src):
+        """[N_r, N_r_src] matrix of the degree-8 Lagrange interpolation from the radial nodes of oracle ``src`` to
+        the nodes of this one (R18): row j holds the nine basis values l_q(r_j) = prod_{p != q} (r_j - x_p) / (x_q - x_p)
+        on the source nodes x = r_src[s..s+8], s = clamp(c - 4, 0, N_src - 9), c = the source node nearest to r_j
+        (the lower one on a tie).  Extended precision, rounded once."""
+        xs = src.r.astype(LD)
+        W = np.zeros((self.p.N_r, src.p.N_r), LD)
+        for j, rj in enumerate(self.r.astype(LD)):
+            c = int(np.argmin(np.abs(src.r.astype(np.float64) - np.float64(rj))))
+            s = min(max(c - 4, 0), src.p.N_r - 9)
+            x = xs[s:s + 9]
+            for q in range(9):
+                num = den = LD(1)
+                for pp in range(9):
+                    if pp != q:
+                        num = num * (rj - x[pp])
+                        den = den * (x[q] - x[pp])
+                W[j, s + q] = num / den
+        return W.astype(self.real)
+
+    def regrid(self, state, src):
+        """State of oracle ``src`` carried onto this oracle's radial grid and mode set ("At every
+        restart, the spatial resolution can be changed using an automated interpolation and mode padding
+        functionality"; R18): radial interpolation by ``regrid_matrix``; modes the source does not hold are zero,
+        modes this oracle does not hold are dropped.  T is dropped if this oracle has no temperature."""
+        p, q = self.p, src.p
+        assert (p.eta, p.alpha, p.k_theta0) == (q.eta, q.alpha, q.k_theta0) and (q.heated or not p.heated)
+        W = self.regrid_matrix(src)
+        Mc, Kc = min(p.M, q.M), min(p.K, q.K)
+        out = []
+        for i, f in enumerate(state):
+            if f is None or (i == 3 and not p.heated):
+                out.append(None)
+                continue
+            g = self.zeros()
+            part = f[:, :Mc + 1, q.K - Kc:q.K + Kc + 1]
+            g[:, :Mc + 1, p.K - Kc:p.K + Kc + 1] = np.einsum("jl,lmk->jmk", W, part)
+            out.append(g)
+        return out
+
     # ---------------------------------------------------------------- NEXT-3: wave speed
     def wave_speed(self, state, field, j, m, k, dt, n_steps):
         """Angular phase speed of one Fourier coefficient f^(r_j; m, k) ~ e^{i (n theta - omega t)} over n_steps

@@ -22,7 +22,7 @@ EXPORTS = (
     "nsc_set_state", "nsc_get_state", "nsc_set_state_host", "nsc_get_state_host",
     "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_step_iterated", "nsc_nusselt", "nsc_probe", "nsc_last_error", "nsc_device_bytes",
     "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name", "nsc_graph_replays",
-    "nsc_fp64_peak", "nsc_cfl_rate", "nsc_advance", "nsc_mode_coefficient", "nsc_wave_speed",
+    "nsc_fp64_peak", "nsc_cfl_rate", "nsc_advance", "nsc_mode_coefficient", "nsc_wave_speed", "nsc_regrid",
 )
 NSC_NKERN = 11
 
@@ -97,6 +97,7 @@ def load_library() -> C.CDLL:
     lib.nsc_advance.argtypes = [vp, dbl, i32, dbl, dbl, dbl, i32, C.POINTER(nsc_advance_info), C.POINTER(dbl)]
     lib.nsc_mode_coefficient.argtypes = [vp, i32, i32, i32, i32, C.POINTER(dbl)]
     lib.nsc_wave_speed.argtypes = [vp, i32, i32, i32, i32, dbl, i32, C.POINTER(dbl)]
+    lib.nsc_regrid.argtypes = [vp, vp]
     for name in EXPORTS:
         if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count", "nsc_kernel_name",
                         "nsc_graph_replays"):
@@ -251,6 +252,10 @@ class Context:
         v = C.c_double(0.0)
         self._check(self._lib.nsc_wave_speed(self._h, field, j, m, k, dt, n_steps, C.byref(v)))
         return v.value
+
+    def regrid_from(self, src: "Context"):
+        """nsc_regrid: this context's state := src's state interpolated / padded onto this resolution."""
+        self._check(self._lib.nsc_regrid(self._h, src._h))
 
     def step(self, dt):
         self._check(self._lib.nsc_step(self._h, float(dt)))

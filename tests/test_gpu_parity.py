@@ -624,3 +624,42 @@ def test_wave_speed_matches_oracle(torch_cuda):
         ctx.set_state(*_dev(torch, st))
         got = ctx.wave_speed(1, 12, 1, 2, cfg["dt"], 5)
     assert abs(got - ref) <= 1e-8 * abs(ref)
+
+
+@pytest.mark.parametrize("src,dst", [((0, 20, 4, 8, 1), (0, 33, 8, 4, 0)), ((2, 24, 8, 8, 1), (2, 16, 4, 16, 1)),
+                                     ((2, 18, 4, 4, 0), (0, 18, 4, 4, 0))])
+def test_regrid_matches_oracle(torch_cuda, src, dst):
+    """NEXT-4 (R18): nsc_regrid against the oracle's regrid -- radial interpolation onto another
+    grid family and node count, mode padding and truncation, pressure included, temperature kept or dropped;
+    regridding onto the same resolution is the identity; the regridded context steps on in parity."""
+    torch = torch_cuda
+    ca = dict(synth.scaled_config(src[0], N_r=src[1], M=src[2], K=src[3]), grid=src[4])
+    cb = dict(synth.scaled_config(dst[0], N_r=dst[1], M=dst[2], K=dst[3]), grid=dst[4])
+    for key in ("eta", "alpha", "k_theta0"):
+        cb[key] = ca[key]
+    oa, ob = oracle_of(ca, dft="fft"), oracle_of(cb, dft="fft")
+    nfb = nf_of(cb)
+    st = synth.make_state(ca, oa.r)
+    rng = np.random.default_rng(7)
+    st[4] = 3.0 * (rng.standard_normal(st[0].shape) + 1j * rng.standard_normal(st[0].shape))
+    ref = ob.regrid(st, oa)
+    with _ctx(ca) as a, _ctx(cb) as b, _ctx(ca) as a2:
+        with pytest.raises(Exception):
+            b.regrid_from(a)                         # the source has no state yet
+        a.set_state(*_dev(torch, st))
+        b.regrid_from(a)
+        got = b.state_to_host()
+        for g, r_ in zip(got, ref):
+            assert (g is None) == (r_ is None)
+        keep = [i for i in range(5) if ref[i] is not None]
+        scale = max(np.abs(ref[i]).max() for i in keep)
+        for i in keep:
+            assert np.abs(got[i] - ref[i]).max() <= 1e-13 * scale
+            assert np.array_equal(got[i] == 0, ref[i] == 0)      # padded modes are exactly zero
+        a2.regrid_from(a)                            # same resolution: the identity
+        for g, s_ in zip(a2.state_to_host(), st):
+            if s_ is not None:
+                np.testing.assert_array_equal(g, s_)
+        b.step(cb["dt"])
+        nxt = b.state_to_host()
+    check_parity(nxt[:nfb], ob.step(ref, cb["dt"])[:nfb], TOL_STEP, cb["K"], "one step after the regrid")

@@ -124,3 +124,83 @@ def test_wave_speed_of_a_scalar_carried_by_solid_body_rotation(m, k):
     assert errs[1] <= 3e-4
     assert 3.8 <= errs[0] / errs[1] <= 4.2                         # second order in dt
     assert abs((4 * sp[1] - sp[0]) / 3 - Omega) <= 1e-5 * Omega    # Richardson limit dt -> 0: exactly Omega
+
+
+# ------------------------------------------------------------------ NEXT-4: restart on another resolution (R18)
+def _pair(N_src, M_src, K_src, grid_src, N_dst, M_dst, K_dst, grid_dst, ci=0):
+    a = dict(synth.scaled_config(ci, N_r=N_src, M=M_src, K=K_src), grid=grid_src)
+    b = dict(synth.scaled_config(ci, N_r=N_dst, M=M_dst, K=K_dst), grid=grid_dst)
+    return a, b, oracle_of(a, dft="fft"), oracle_of(b, dft="fft")
+
+
+@pytest.mark.parametrize("grids", [(1, 1), (1, 0), (0, 1)])
+def test_regrid_is_exact_for_polynomials_of_degree_8_and_pads_modes(grids):
+    """Radial interpolation reproduces r^p, p <= 8, to round-off on any pair of grids (and not r^9); modes the
+    source does not hold come out zero, modes the target does not hold are dropped, shared modes keep their place."""
+    ca, cb, oa, ob = _pair(20, 4, 8, grids[0], 33, 8, 4, grids[1])
+    K_a, K_b = 8, 4
+    st = [oa.zeros() for _ in range(3)] + [None, oa.zeros()]
+    for p in range(10):
+        for f in st:
+            if f is not None:
+                f[...] = 0
+        st[1][:, 2, K_a + 3] = (1 + 2j) * oa.r ** p          # (m, k) = (2, 3): held by both
+        st[1][:, 3, K_a - 7] = oa.r ** p                     # k = -7: not held by the target (K = 4)
+        st[4][:, 0, K_a] = oa.r ** p
+        out = ob.regrid(st, oa)
+        err = np.abs(out[1][:, 2, K_b + 3] - (1 + 2j) * ob.r ** p).max() / (ob.r[-1] ** p)
+        errp = np.abs(out[4][:, 0, K_b] - ob.r ** p).max() / (ob.r[-1] ** p)
+        if p <= 8:
+            assert err <= 5e-14 and errp <= 5e-14
+        else:
+            assert err > 1e-11
+        assert out[3] is None and out[0].shape == (33, 9, 9)
+        mask = np.ones(out[1].shape, bool)
+        mask[:, 2, K_b + 3] = False
+        assert np.all(out[1][mask] == 0)                     # k = -7 dropped, m = 5..8 padded with zeros
+
+
+def test_regrid_onto_the_same_grid_is_the_identity_and_nodes_in_common_keep_their_values():
+    ca, cb, oa, ob = _pair(17, 4, 4, 0, 33, 4, 4, 0)        # uniform grids: every second fine node is a coarse node
+    st = synth.make_state(ca, oa.r)
+    same = oa.regrid(st, oa)
+    for a, b in zip(same, st):
+        if b is not None:
+            np.testing.assert_array_equal(a, b)
+    fine = ob.regrid(st, oa)
+    np.testing.assert_allclose(ob.r[::2], oa.r, rtol=0, atol=1e-15)
+    for a, b in zip(fine, st):
+        if b is not None:
+            np.testing.assert_allclose(a[::2], b, rtol=0, atol=1e-13 * np.abs(b).max())
+    W = ob.regrid_matrix(oa)
+    np.testing.assert_allclose(W.sum(axis=1), 1.0, rtol=0, atol=1e-13)       # partition of unity
+    assert np.count_nonzero(W[5]) <= 9
+
+
+def test_regrid_interpolation_error_falls_at_ninth_order():
+    errs = []
+    for N in (12, 24, 48):
+        ca, cb, oa, ob = _pair(N, 4, 4, 0, 101, 4, 4, 0)
+        st = [oa.zeros() for _ in range(3)] + [None, None]
+        st[0][:, 1, 4] = np.exp(1.3 * oa.r) * np.sin(2.0 * oa.r)
+        out = ob.regrid(st, oa)
+        errs.append(np.abs(out[0][:, 1, 4] - np.exp(1.3 * ob.r) * np.sin(2.0 * ob.r)).max())
+    assert errs[0] / errs[1] >= 2 ** 8 and errs[1] / errs[2] >= 2 ** 8 or errs[2] <= 1e-13
+
+
+def test_a_regridded_flow_keeps_running():
+    """Restart of cfg 1 on a finer resolution: the interpolated state is divergence-free to interpolation accuracy,
+    one step later to round-off again, and the coarse and the fine run agree on the shared modes."""
+    ca, cb, oa, ob = _pair(24, 8, 8, 1, 32, 8, 8, 1)
+    st = synth.make_state(ca, oa.r)
+    for _ in range(2):
+        st = oa.step(st, ca["dt"])
+    fine = ob.regrid(st, oa)
+    d0 = np.abs(ob.divergence(*fine[:3])[1:-1]).max()
+    nxt = ob.step(fine, cb["dt"])
+    d1 = np.abs(ob.divergence(*nxt[:3])[1:-1]).max()
+    scale = np.abs(ob.D1) @ np.abs(nxt[1][:, 0, 8])
+    assert d0 <= 1e-6 * scale.max() and d1 <= 1e-11 * scale.max()
+    ref = oa.step(st, ca["dt"])
+    back = oa.regrid(nxt, ob)
+    assert rel_l2(back[:3], ref[:3]) <= 5e-6          # interpolation accuracy at these resolutions
