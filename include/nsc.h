@@ -49,17 +49,18 @@ enum {
 /* Extended creation parameters (nsc_create fills the defaults marked below). */
 typedef struct nsc_params {
     int N_r;          /* radial nodes, >= 9 (9-point stencil)                      */
-    int M_theta;      /* azimuthal modes m = 0..M_theta; M_theta in {4,8,...,512} (power of two)  */
-    int K_z;          /* axial modes k = -K_z..K_z;     K_z in {4,8,...,512} (power of two)       */
+    int M_theta;      /* azimuthal modes m = 0..M_theta, 1 <= M_theta <= 512                       */
+    int K_z;          /* axial modes k = -K_z..K_z,     1 <= K_z <= 512                            */
     double eta;       /* radius ratio r_i / r_o, 0 < eta < 1                                      */
     double alpha;     /* axial base wavenumber (domain length 2 pi / alpha), > 0                  */
     int k_theta0;     /* azimuthal base wavenumber, >= 1                                          */
     double Re_i, Re_o;/* inner / outer wall speed (units nu/d)                                    */
     double Ra, Pr;    /* Rayleigh, Prandtl number; Ra == 0 switches temperature off; Pr > 0       */
     int radial_grid;  /* 0 uniform, 1 Chebyshev-Gauss-Lobatto clustering (R2)                     */
-    int n_theta_phys; /* physical grid points in theta; 0 => 3 M_theta (3/2 rule, R4)             */
-    int n_z_phys;     /* physical grid points in z;     0 => 3 K_z; allowed: 3*2^p or 6*2^p lengths
-                         in {12,24,...,1536} that are >= the 3/2 rule                              */
+    int n_theta_phys; /* physical grid points in theta; 0 => the shortest supported length >= 3 M_theta
+                       * (3/2 rule, R4; = 3 M_theta when M_theta is a power of two >= 4)           */
+    int n_z_phys;     /* physical grid points in z;     0 => likewise for K_z.  Supported transform
+                       * lengths: 3 * 2^p in {12, 24, ..., 1536}; a given length must be >= the 3/2 rule */
     double c;         /* implicitness of the linear terms; 0 => 0.5 (R10)                         */
     int device;       /* CUDA device ordinal; -1 => current device                                */
     int radial_chunk; /* radial nodes per pass of the transform pipeline; 0 => automatic (all N_r

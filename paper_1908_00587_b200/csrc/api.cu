@@ -73,8 +73,6 @@ static const char* kKernelNames[NSC_NKERN] = {"k_zinv", "k_theta", "k_zfwd", "k_
                                               "k_diff_norm", "k_nusselt / k_probe", "k_poisson_fwd", "k_poisson_bwd_correct",
                                               "k_factor", "k_dr"};
 
-static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
-
 }  // namespace nsc
 
 using namespace nsc;
@@ -85,15 +83,21 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
     if (!out || !pp) return fail(nullptr, NSC_EINVAL, "nsc_create: NULL argument");
     nsc_params p = *pp;
     if (p.N_r < NPT) return fail(nullptr, NSC_EINVAL, "nsc_create: N_r must be >= 9");
-    if (!pow2_in(p.M_theta, 4, 512) || !pow2_in(p.K_z, 4, 512))
-        return fail(nullptr, NSC_EINVAL, "nsc_create: M_theta and K_z must be powers of two in [4, 512]");
+    if (p.M_theta < 1 || p.M_theta > 512 || p.K_z < 1 || p.K_z > 512)
+        return fail(nullptr, NSC_EINVAL, "nsc_create: M_theta and K_z must be in [1, 512]");
     if (!(p.eta > 0.0 && p.eta < 1.0)) return fail(nullptr, NSC_EINVAL, "nsc_create: eta must be in (0, 1)");
     if (!(p.alpha > 0.0)) return fail(nullptr, NSC_EINVAL, "nsc_create: alpha must be > 0");
     if (p.k_theta0 < 1) return fail(nullptr, NSC_EINVAL, "nsc_create: k_theta0 must be >= 1");
     if (p.Ra != 0.0 && !(p.Pr > 0.0)) return fail(nullptr, NSC_EINVAL, "nsc_create: Pr must be > 0 when Ra != 0");
     if (p.radial_grid != 0 && p.radial_grid != 1) return fail(nullptr, NSC_EINVAL, "nsc_create: radial_grid must be 0 or 1");
-    if (p.n_theta_phys == 0) p.n_theta_phys = 3 * p.M_theta;
-    if (p.n_z_phys == 0) p.n_z_phys = 3 * p.K_z;
+    // default physical grid: the shortest supported transform length (3 * 2^p, 12..1536) that holds the 3/2 rule
+    auto default_len = [](int modes) {
+        int n = 12;
+        while (n < 3 * modes) n *= 2;
+        return n;
+    };
+    if (p.n_theta_phys == 0) p.n_theta_phys = default_len(p.M_theta);
+    if (p.n_z_phys == 0) p.n_z_phys = default_len(p.K_z);
     if (p.n_theta_phys < 3 * p.M_theta || p.n_z_phys < 3 * p.K_z || !fft_length_supported(p.n_theta_phys) ||
         !fft_length_supported(p.n_z_phys))
         return fail(nullptr, NSC_EINVAL, "nsc_create: unsupported physical grid size");

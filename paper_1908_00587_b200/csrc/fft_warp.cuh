@@ -1,4 +1,5 @@
-// fft_warp.cuh -- two-pass fp64 FFTs of length N = NA x 32 (NA = 24: N = 768, NA = 12: N = 384) for one warp.
+// fft_warp.cuh -- two-pass fp64 FFTs of length N = NA x 32 (NA = 24: N = 768, NA = 12: N = 384) for one warp,
+// and of length 1536 = 2 x 768 for a pair of warps.
 //
 // The long workloads (BASELINE.json configs[3]: 768 x 768 physical grid per radial node, configs[2]: 384 x 384)
 // spend their time in these transforms.  With 24 complex values per thread the generic
@@ -195,6 +196,66 @@ template <int NA, int DIR> __device__ __forceinline__ void p2s(cd* x, cd* buf, c
     p2s_front<DIR>(x, buf, tw, tau < NV ? tau : NV - 1, tau < NV);
     __syncwarp();
     p2s_back<NA, DIR>(x, buf, tau);
+}
+
+// ---------------------------------------------------------------- length 1536 = 2 x 768 on a warp pair
+// Warp h (= 0, 1) of a pair holds the samples of parity h in the S layout (register t of lane tau: index
+// h + 2 (tau + 32 t)) and, on the P side, the half h of the line (lane a, register e: index a + 24 p(e) + 768 h).
+// s2p_pair: each warp transforms its decimated sequence (E, O), then X[k'] = E + W^k' O, X[k' + 768] = E - W^k' O
+// (decimation in time); p2s_pair is the mirror image (decimation in frequency: sums to the even outputs, twiddled
+// differences to the odd ones).  The halves meet through the warps' exchange matrices (row a, column e) under a
+// named barrier of the 64 threads of the pair.  twc[k'] = exp(-2 pi i k' / 1536), k' < 768.
+constexpr int NPAIR = 1536;
+__device__ __forceinline__ void pair_sync(int pair) { asm volatile("bar.sync %0, 64;" ::"r"(1 + pair) : "memory"); }
+
+template <int DIR>
+__device__ __forceinline__ void s2p_pair(cd* x, cd* buf, const cd* pbuf, const cd* tw, const cd* twc, int tau, int h,
+                                         int pair) {
+    const int a = tau < NV ? tau : NV - 1;
+    pair_sync(pair);                   // the partner has finished reading my matrix (previous combine)
+    s2p<24, DIR>(x, buf, tw, tau);
+    if (h == 1) {
+#pragma unroll
+        for (int e = 0; e < NB; ++e) {
+            cd w = twc[a + NV * p_of(e)];
+            if (DIR > 0) w = conj(w);
+            x[e] = x[e] * w;
+        }
+    }
+    __syncwarp();                      // every lane has read its row of the matrix
+    if (tau < NV)
+#pragma unroll
+        for (int e = 0; e < NB; ++e) buf[a * XS + e] = x[e];
+    pair_sync(pair);
+#pragma unroll
+    for (int e = 0; e < NB; ++e) {
+        const cd y = pbuf[a * XS + e];
+        x[e] = h == 0 ? x[e] + y : y - x[e];
+    }
+}
+
+template <int DIR>
+__device__ __forceinline__ void p2s_pair(cd* x, cd* buf, const cd* pbuf, const cd* tw, const cd* twc, int tau, int h,
+                                         int pair) {
+    const int a = tau < NV ? tau : NV - 1;
+    pair_sync(pair);                   // both matrices are free
+    if (tau < NV)
+#pragma unroll
+        for (int e = 0; e < NB; ++e) buf[a * XS + e] = x[e];
+    pair_sync(pair);
+#pragma unroll
+    for (int e = 0; e < NB; ++e) {
+        const cd y = pbuf[a * XS + e];
+        if (h == 0) {
+            x[e] = x[e] + y;
+        } else {
+            cd w = twc[a + NV * p_of(e)];
+            if (DIR > 0) w = conj(w);
+            x[e] = (y - x[e]) * w;
+        }
+    }
+    pair_sync(pair);                   // the partner has read my matrix: the transform may overwrite it
+    p2s<24, DIR>(x, buf, tw, tau);
 }
 
 // cooperative copy of the [24][33] twiddle matrix (global, plan.cu) into shared memory

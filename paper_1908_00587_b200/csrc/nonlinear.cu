@@ -67,6 +67,8 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
     Nl2Args a2{};
     a2.tw_z = c->t.tw_wz;
     a2.tw_t = c->t.tw_wt;
+    a2.tw_cz = c->t.tw_c1536;
+    a2.tw_ct = c->t.tw_c1536;
     a2.alpha = c->p.alpha;
     a2.ktheta0 = (double)c->p.k_theta0;
     // N1, radial derivative.  One radial chunk (JC = N_r): D1 is applied to the z-transformed fields inside the

@@ -19,6 +19,8 @@ struct Nl2Args {
     const cd* dr[MAXF];    // radial derivatives of the input fields, spectral layout
     const cd* tw_z;        // [24][33] twiddle matrix of fft_warp.cuh for the z length (plan.cu)
     const cd* tw_t;        // ... for the theta length
+    const cd* tw_cz;       // [768] exp(-2 pi i k / 1536): combine twiddles of the warp-pair transform (length 1536), z
+    const cd* tw_ct;       // ... theta
     double alpha;          // axial base wavenumber
     double ktheta0;        // azimuthal base wavenumber
     int nitems;            // work items of the launch
@@ -26,7 +28,8 @@ struct Nl2Args {
 
 // host-side launchers (nonlinear_v2.cu)
 int launch_dr(const DrArgs& a, int nf, cudaStream_t st);
-// na = 24 (length 768) or 12 (length 384); warp_na(n, modes): the na of length n if the warp kernels serve it
+// na = 24 (length 768), 12 (length 384) or 48 (length 1536 = 2 x 768 on warp pairs, nonlinear_v3.cuh);
+// warp_na(n, modes): the na of length n if the warp kernels serve it, else 0
 int warp_na(int n, int modes);
 int warp_mtile(int na);    // m-lines per work item of the z kernels
 int launch_zinv2(int na, const Nl2Args& a, cudaStream_t st);

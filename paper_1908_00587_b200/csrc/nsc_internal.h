@@ -45,6 +45,7 @@ struct Tables {               // all device pointers
     cd* tw_z = nullptr;       // [N_z]
     cd* tw_wz = nullptr;      // [24][33]   twiddle matrix of fft_warp.cuh for N_z (if its length is 768 or 384)
     cd* tw_wt = nullptr;      // [24][33]   ... for N_theta
+    cd* tw_c1536 = nullptr;   // [768]      exp(-2 pi i k / 1536): combine twiddles of the warp-pair transform (length 1536)
 };
 
 }  // namespace nsc
@@ -76,7 +77,7 @@ struct nsc_ctx {
     nsc::cd* zbuf = nullptr;              // [JC][3 nf][N_z][MP]  z-transformed f, dz f, dr f
     nsc::cd* tbuf = nullptr;              // [JC][nf][N_z][MP]    theta-transformed products
     nsc::cd* DR[nsc::MAXF] = {nullptr, nullptr, nullptr, nullptr};       // D1 f (warp z pipeline in several chunks)
-    int z_na = 0;                         // z transforms by k_dr + k_zinv2 / k_zfwd2 of fft_warp.cuh: 24 (768), 12 (384), 0 no
+    int z_na = 0;                         // z transforms by k_dr + k_zinv2 / k_zfwd2 of fft_warp.cuh: 24 (768), 12 (384), 48 (1536, warp pairs), 0 no
     int t_na = 0;                         // theta transforms by k_theta2: 24, 12, 0 no
     unsigned long long* cfl_max = nullptr;    // [N_r][3] per-level maxima of |u| (k_theta2 / k_theta), step-size control
     bool want_cfl = false;                // the next launch_nonlinear accumulates them

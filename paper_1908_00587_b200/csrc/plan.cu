@@ -163,6 +163,7 @@ int build_plan(nsc_ctx* c) {
     if ((rc = upload(c, &c->t.tw_z, twiddles(c->Nz)))) return rc;
     // twiddle matrices of the warp transforms (fft_warp.cuh): tw[t][n2] = exp(-2 pi i (t % NA) n2 / N), row stride 33
     auto warp_table = [&](int n, cd** dst) -> int {
+        if (n == fw::NPAIR) n /= 2;                      // a warp pair runs two transforms of length 768
         const int na = n / fw::NB;
         std::vector<cd> t(fw::XBUF, mk(0.0, 0.0));
         for (int r = 0; r < fw::NV; ++r)
@@ -174,6 +175,14 @@ int build_plan(nsc_ctx* c) {
     };
     if (c->z_na && (rc = warp_table(c->Nz, &c->t.tw_wz))) return rc;
     if (c->t_na && (rc = warp_table(c->Nt, &c->t.tw_wt))) return rc;
+    if (c->z_na == 48 || c->t_na == 48) {
+        std::vector<cd> t(fw::NPAIR / 2);
+        for (int k = 0; k < fw::NPAIR / 2; ++k) {
+            ld a = 2 * pi_ld() * (ld)k / fw::NPAIR;
+            t[k] = mk((double)cosl(a), (double)(-sinl(a)));
+        }
+        if ((rc = upload(c, &c->t.tw_c1536, t))) return rc;
+    }
 
     // ---- band envelopes.  Helmholtz: identity rows at the walls (Dirichlet), stencil rows inside.
     c->shH.h_lo.resize(N);

@@ -31,7 +31,8 @@ def test_bad_arguments_are_rejected_before_touching_a_device(lib):
     from paper_1908_00587_b200 import nsc
     h = C.c_void_p()
     bad = [
-        dict(N_r=8), dict(M_theta=6), dict(K_z=3), dict(eta=1.5), dict(alpha=-1.0), dict(k_theta0=0),
+        dict(N_r=8), dict(M_theta=0), dict(K_z=513), dict(K_z=8, n_z_phys=36), dict(eta=1.5), dict(alpha=-1.0),
+        dict(k_theta0=0),
         dict(radial_grid=2), dict(Ra=10.0, Pr=0.0), dict(n_z_phys=20), dict(n_theta_phys=12),
     ]
     for over in bad:

@@ -69,6 +69,8 @@ NL_CASES = [
     (4, 9, 512, 4, "naive"),      # heated; 1536 / 12 (cfg 5's theta length)
     (4, 9, 4, 512, "naive"),      # heated; 12 / 1536
     (2, 10, 128, 128, "naive"),   # heated; 384 / 384 (cfg 3's lengths)
+    (4, 9, 512, 512, "naive"),    # heated; 1536 / 1536 (cfg 5's lengths: warp-pair kernels in both directions)
+    (3, 9, 512, 8, "naive"),      # no temperature; 1536 / 24
 ]
 
 
@@ -100,7 +102,7 @@ def test_nonlinear_length_768_kernels_on_a_padded_grid(torch_cuda, ci, N_r, M, K
     check_parity(got, o.nonlinear(*st[:3]), TOL_N, K, f"nonlinear {N_r}x{M}x{K} on {n_theta or 3 * M} x {n_z or 3 * K}")
 
 
-@pytest.mark.parametrize("ci,N_r,M,K", [(3, 9, 256, 256), (2, 9, 128, 128)])
+@pytest.mark.parametrize("ci,N_r,M,K", [(3, 9, 256, 256), (2, 9, 128, 128), (3, 9, 512, 512)])
 def test_nonlinear_white_noise_through_the_long_transforms(torch_cuda, ci, N_r, M, K):
     """Full-band white-noise fields with a non-Hermitian m = 0 row (reading R6) through the length-768 and
     length-384 kernels, against the naive-DFT oracle."""
@@ -113,6 +115,28 @@ def test_nonlinear_white_noise_through_the_long_transforms(torch_cuda, ci, N_r, 
         ctx.set_state(*(_dev(torch, fs) + [None] * (5 - nf)))
         got = ctx.nonlinear_to_host()
     check_parity(got, o.nonlinear(*fs), TOL_N, K, f"white-noise nonlinear {N_r}x{M}x{K}")
+
+
+@pytest.mark.parametrize("ci,N_r,M,K,n_theta,n_z", [(0, 12, 5, 6, 24, 24), (2, 10, 100, 50, 384, 192), (1, 9, 1, 3, 12, 12)])
+def test_mode_counts_that_are_not_powers_of_two(torch_cuda, ci, N_r, M, K, n_theta, n_z):
+    """Any 1 <= M, K <= 512: the default physical grid is the shortest supported transform length that holds the
+    3/2 rule; nonlinear term and two steps against the oracle on that grid."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    nf = nf_of(cfg)
+    o = oracle_of(cfg, dft="fft", n_theta=n_theta, n_z=n_z)
+    with _ctx(cfg) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        got = ctx.nonlinear_to_host()
+        check_parity(got, o.nonlinear(*st[:nf]), TOL_N, K, f"nonlinear {N_r}x{M}x{K} on the default grid")
+        for _ in range(2):
+            ctx.step(cfg["dt"])
+        end = ctx.state_to_host()
+    ref = st
+    for _ in range(2):
+        ref = o.step(ref, cfg["dt"])
+    check_parity(end[:nf], ref[:nf], TOL_STEP, K, f"two steps {N_r}x{M}x{K}")
 
 
 def test_nonlinear_broadband_random_fields_and_chunking(torch_cuda):
@@ -424,7 +448,8 @@ def test_diagnostics_match_oracle(torch_cuda, ci, N_r, M, K):
             ctx.probe(3 if nf == 3 else 5, 0, 0.0, 0.0)
 
 
-@pytest.mark.parametrize("ci,N_r,M,K,chunk", [(1, 10, 8, 256, 4), (3, 12, 256, 8, 5), (3, 11, 256, 256, 3)])
+@pytest.mark.parametrize("ci,N_r,M,K,chunk", [(1, 10, 8, 256, 4), (3, 12, 256, 8, 5), (3, 11, 256, 256, 3), (1, 10, 8, 512, 3),
+                                             (1, 10, 8, 128, 4)])
 def test_nonlinear_length_768_in_several_radial_chunks(torch_cuda, ci, N_r, M, K, chunk):
     """The multi-chunk form of the length-768 pipeline (spectral k_dr + three z transforms per line, used when
     the work arrays of the whole radius do not fit) against the oracle, and against the single-chunk form."""
@@ -541,7 +566,8 @@ def test_graph_replay_after_a_substep_with_another_dt(torch_cuda):
             np.testing.assert_array_equal(a, b)
 
 
-@pytest.mark.parametrize("ci,N_r,M,K", [(0, 20, 4, 4), (2, 12, 16, 32), (1, 11, 64, 8), (3, 9, 256, 256), (2, 10, 128, 128)])
+@pytest.mark.parametrize("ci,N_r,M,K", [(0, 20, 4, 4), (2, 12, 16, 32), (1, 11, 64, 8), (3, 9, 256, 256), (2, 10, 128, 128),
+                                       (4, 9, 512, 16)])
 def test_cfl_rate_matches_oracle(torch_cuda, ci, N_r, M, K):
     """NEXT-1 (R17): nsc_cfl_rate (maxima of |u| per radial level gathered inside the theta kernels, generic and
     warp-transform forms) against the oracle's cfl_rate on the physical grid."""
