@@ -450,13 +450,27 @@ def run_ours(args, cfg, rank, world, local_rank):
     launches_dom = dom.get("launches_per_step", None)
     traffic, traffic_src = ncu_traffic(dom["kernel"], args.config)
     for k in kern:
-        k["bound"] = "fp64" if k["kernel"] == "k_theta" else "hbm"
-    roofline = {
-        "bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_GBs"], "peak": peak, "unit": "GB/s",
-        "frac": dom["achieved_GBs"] / peak, "peak_source": peak_src,
-        "note": ("the dominant kernel's algorithmic bytes over its time against the HBM copy peak; that kernel (the fused "
-                 "theta transforms) is bound by the fp64 pipe, see 'alu'; the step-level HBM fraction is 'step'"
-                 if dom["kernel"] == "k_theta" else None),
+        k["bound"] = "alu" if k["kernel"] == "k_theta" else "hbm"
+    th = next((k for k in kern if k["kernel"] == "k_theta"), None)
+    hbm_view = {"achieved": dom["achieved_GBs"], "peak": peak, "unit": "GB/s", "frac": dom["achieved_GBs"] / peak,
+                "peak_source": peak_src}
+    if dom["kernel"] == "k_theta":
+        # the dominant kernel (the fused theta transforms) is bound by the plain fp64 pipe, not by HBM: its model flops
+        # (5 N log2 N per complex transform + the products) over its time against the fp64 peak MEASURED in this run
+        flops = 2 * flops_theta_per_nonlinear(cfg)
+        tf = flops / 1e9 / th["ms_per_step"]
+        head = {"bound": "alu", "kernel": "k_theta", "achieved": tf, "peak": fp64_fma, "unit": "TFLOP/s",
+                "frac": tf / fp64_fma,
+                "peak_source": "measured: nsc_fp64_peak(kind 0): register-only DFMA kernel on every SM, 2 flop per instruction",
+                "note": ("fp64 butterflies are mostly additions and multiplications that cannot fuse; against the measured "
+                         "DADD+DMUL rate (1 flop per instruction) the same flops are frac_of_addmul_peak"),
+                "addmul_peak": fp64_addmul, "frac_of_addmul_peak": tf / fp64_addmul,
+                "nominal_dfma_peak": FP64_NOMINAL_TFLOPS,
+                "hbm_view": hbm_view}
+    else:
+        head = dict(hbm_view, bound="hbm", kernel=dom["kernel"])
+    roofline = dict(head)
+    roofline.update({
         "traffic": traffic, "traffic_source": traffic_src,
         "share_of_step": dom["share"],
         "algorithmic_bytes_per_launch": (model.get(dom["kernel"], model["linear"]) / launches_dom
@@ -465,22 +479,10 @@ def run_ours(args, cfg, rank, world, local_rank):
         "step": {"algorithmic_GB": model["step"] / 1e9, "achieved_GBs": model["step"] / 1e6 / ms_per_step,
                  "frac_of_measured": model["step"] / 1e6 / ms_per_step / peak,
                  "frac_of_nominal_8TBs": model["step"] / 1e6 / ms_per_step / NOMINAL_HBM_GBS},
-        "fp64": {"GF_per_nonlinear": flops_per_nonlinear(cfg) / 1e9},
-        # the theta kernel is co-bound by the plain fp64 pipe: its own ALU roofline
-        # the theta kernel is bound by the plain fp64 pipe: its flops (model: 5 N log2 N per complex transform, mostly
-        # additions and multiplications that do not fuse) against the measured DADD+DMUL rate and the DFMA rate
-        "alu": ({"bound": "fp64", "kernel": "k_theta",
-                 "achieved": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"],
-                 "peak": fp64_addmul, "unit": "TFLOP/s",
-                 "frac": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"] / fp64_addmul,
-                 "peak_source": "measured: nsc_fp64_peak(kind 1, DADD + DMUL alternating, 1 flop per instruction)",
-                 "peak_dfma": fp64_fma, "frac_of_dfma_peak": 2 * flops_theta_per_nonlinear(cfg) / 1e9 / th["ms_per_step"] / fp64_fma,
-                 "peak_dfma_source": "measured: nsc_fp64_peak(kind 0, DFMA only, 2 flop per instruction)",
-                 "nominal_dfma_peak": FP64_NOMINAL_TFLOPS}
-                if (th := next((k for k in kern if k["kernel"] == "k_theta"), None)) else None),
+        "fp64": {"GF_per_nonlinear": flops_per_nonlinear(cfg) / 1e9, "dfma_peak_TFLOPs": fp64_fma, "addmul_peak_TFLOPs": fp64_addmul},
         "kernels": kern + [lin],
         "ms_per_step_with_event_brackets": ms_prof_per_step,
-    }
+    })
     value = replicas.aggregate_rate(world, args.steps, ms / 1e3)
     mode_points = s["N_r"] * (s["M"] + 1) * (2 * s["K"] + 1)
     nbytes_state = len(names) * F

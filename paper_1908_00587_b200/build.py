@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnsc.so")
-FFT_LENGTHS = (12, 24, 48, 96, 192, 384, 768, 1536)
+FFT_LENGTHS = (12, 24, 48, 96, 192)          # generic kernels; 384, 768, 1536: warp-transform kernels (nonlinear_v2.cu)
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -130,24 +130,9 @@ __device__ __forceinline__ cd ldcs(const cd* p) {
 
 // ---- row pipeline: every row's operands arrive in shared memory by cp.async, PIPE - 1 rows ahead of
 // the row being eliminated, so that the marching threads never wait on HBM with a single row in flight
-#ifndef NSC_PBK
-#define NSC_PBK 32
-#endif
-constexpr int PBK = NSC_PBK;     // modes per block
-// shared-memory row slots of the four sweeps (rows in flight = slots - 1)
-#ifndef NSC_PIPE_F
-#define NSC_PIPE_F 3
-#endif
-#ifndef NSC_PIPE_B
-#define NSC_PIPE_B 3
-#endif
-#ifndef NSC_PIPE_PF
-#define NSC_PIPE_PF 3
-#endif
-#ifndef NSC_PIPE_PB
-#define NSC_PIPE_PB 2
-#endif
-constexpr int PIPE_F = NSC_PIPE_F, PIPE_B = NSC_PIPE_B, PIPE_PF = NSC_PIPE_PF, PIPE_PB = NSC_PIPE_PB;
+constexpr int PBK = 32;          // modes per block
+// shared-memory row slots of the four sweeps (rows in flight = slots - 1); measured: more resident blocks beat deeper pipelines
+constexpr int PIPE_F = 3, PIPE_B = 3, PIPE_PF = 3, PIPE_PB = 2;
 __device__ __forceinline__ void cpa16(void* s, const void* g) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(s)), "l"(g) : "memory");
 }
@@ -183,11 +168,8 @@ template <int NF> struct FwdSlot {
     double L[NF][FWI][PBK];
 };
 
-#ifndef NSC_K1_MINB
-#define NSC_K1_MINB 1
-#endif
 template <int NF>
-__global__ void __launch_bounds__(PBK * NF, NSC_K1_MINB) k_rhs_fwd(FusedArgs a) {
+__global__ void __launch_bounds__(PBK * NF, 1) k_rhs_fwd(FusedArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     FwdSlot<NF>* slots = reinterpret_cast<FwdSlot<NF>*>(smem_raw);
     const int tx = threadIdx.x, fld = threadIdx.y;
@@ -326,11 +308,8 @@ template <int NF> struct BwdSlot {
     double U[NF][FWI + 1][PBK];
 };
 
-#ifndef NSC_K2_MINB
-#define NSC_K2_MINB 5
-#endif
 template <int NF>
-__global__ void __launch_bounds__(PBK * (NF + 1), NF == 3 ? NSC_K2_MINB : 3) k_bwd_div(FusedArgs a) {
+__global__ void __launch_bounds__(PBK * (NF + 1), NF == 3 ? 5 : 3) k_bwd_div(FusedArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     BwdSlot<NF>* slots = reinterpret_cast<BwdSlot<NF>*>(smem_raw);
     __shared__ cd exch[2][3][PBK];
@@ -501,14 +480,8 @@ struct PoisArgs {
     double dt;
 };
 
-#ifndef NSC_PBP
-#define NSC_PBP 128
-#endif
-#ifndef NSC_PBB
-#define NSC_PBB 64
-#endif
-constexpr int PBP = NSC_PBP;    // modes per block, forward sweep
-constexpr int PBB = NSC_PBB;    // modes per block, backward sweep + correction
+constexpr int PBP = 128;    // modes per block, forward sweep
+constexpr int PBB = 64;     // modes per block, backward sweep + correction
 constexpr int PW = 16;      // substitution ring (Poisson envelope <= 12)
 constexpr int PWI = 8;      // interior lower / upper width
 

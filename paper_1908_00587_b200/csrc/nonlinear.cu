@@ -10,8 +10,9 @@ struct LenEntry {
     launch_fn zinv, zfwd, theta;
 };
 #define NSC_LEN(N) {N, launch_zinv_##N, launch_zfwd_##N, launch_theta_##N}
-static const LenEntry kLens[] = {NSC_LEN(12), NSC_LEN(24), NSC_LEN(48), NSC_LEN(96),
-                                 NSC_LEN(192), NSC_LEN(384), NSC_LEN(768), NSC_LEN(1536)};
+// generic three-pass kernels (nonlinear_kernels.cuh): the short lengths; 384, 768 and 1536 run the warp-transform
+// kernels of nonlinear_v2.cuh / nonlinear_v3.cuh
+static const LenEntry kLens[] = {NSC_LEN(12), NSC_LEN(24), NSC_LEN(48), NSC_LEN(96), NSC_LEN(192)};
 #undef NSC_LEN
 
 static const LenEntry* find_len(int n) {
@@ -20,7 +21,7 @@ static const LenEntry* find_len(int n) {
     return nullptr;
 }
 
-bool fft_length_supported(int n) { return find_len(n) != nullptr; }
+bool fft_length_supported(int n) { return find_len(n) != nullptr || warp_na(n, 1) != 0; }
 
 int launch_radial_derivative(nsc_ctx* c, const cd* f, cd* out) {
     DrArgs d{};
@@ -39,7 +40,7 @@ int launch_radial_derivative(nsc_ctx* c, const cd* f, cd* out) {
 int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
     const LenEntry* lz = find_len(c->Nz);
     const LenEntry* lt = find_len(c->Nt);
-    if (!lz || !lt) return fail(c, NSC_EINVAL, "unsupported physical grid size");
+    if ((!lz && !c->z_na) || (!lt && !c->t_na)) return fail(c, NSC_EINVAL, "unsupported physical grid size");
     NlArgs a{};
     for (int i = 0; i < c->nf; ++i) {
         a.f[i] = f[i];

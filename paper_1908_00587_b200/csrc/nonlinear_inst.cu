@@ -1,5 +1,5 @@
 // nonlinear_inst.cu -- instantiates the transform kernels for ONE line length, selected with
-// -DNSC_FFT_N=<12|24|48|96|192|384|768|1536>; the build compiles this file once per length
+// -DNSC_FFT_N=<12|24|48|96|192>; the build compiles this file once per length
 // (in parallel) and nonlinear.cu dispatches on the run-time lengths N_theta, N_z.
 #include "nonlinear_kernels.cuh"
 

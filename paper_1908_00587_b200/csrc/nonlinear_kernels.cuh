@@ -410,9 +410,6 @@ NSC_DECLARE_LEN(24)
 NSC_DECLARE_LEN(48)
 NSC_DECLARE_LEN(96)
 NSC_DECLARE_LEN(192)
-NSC_DECLARE_LEN(384)
-NSC_DECLARE_LEN(768)
-NSC_DECLARE_LEN(1536)
 #undef NSC_DECLARE_LEN
 
 }  // namespace nsc
