@@ -325,7 +325,7 @@ def run_ours(args, cfg, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
-    with nsc.Context.from_config(cfg, radial_chunk=args.radial_chunk) as ctx:
+    with nsc.Context.from_config(cfg, radial_chunk=args.radial_chunk, linear_slices=args.linear_slices) as ctx:
         ctx.set_stream(stream)
         st = synth.make_state(replicas.rank_config(cfg, rank), ctx.grid())
         # pinned host copies of the state (inputs of a step) and of the result
@@ -524,6 +524,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--radial-chunk", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--linear-slices", type=int, default=0, help="nsc_params.linear_slices (0: the library's default, 2)")
     ap.add_argument("--extra-configs", type=lambda v: [int(x) for x in v.split(",") if x], default=[3],
                     help="other BASELINE.json configs timed in the same run and reported under other_configs (default 3)")
     args = ap.parse_args()
