@@ -168,6 +168,24 @@ int nsc_mode_coefficient(nsc_ctx* ctx, int field, int j, int m, int k, double* h
  * The state advances by n_steps steps.  Synchronises the stream after every step. */
 int nsc_wave_speed(nsc_ctx* ctx, int field, int j, int m, int k, double dt, int n_steps, double* h_speed);
 
+/* The pieces of a step for a slab-decomposed run over several GPUs (modes are
+ * independent in the linear terms, radial levels in the nonlinear terms).  Every rank holds a
+ * context of the full size and computes only its window; the Python module paper_1908_00587_b200.slabs moves the slabs
+ * between the ranks (torch.distributed) directly inside the library's arrays.
+ *   nsc_set_window     nsc_nonlinear / phases 0, 2 evaluate the radial levels [j0, j0 + nj) only (they read the fields at
+ *                      those levels and four beyond on either side); nsc_substep / phases 1, 3 treat the Fourier modes
+ *                      [e0, e0 + ne) only (flat index m (2 K_z + 1) + k + K_z).  All four arguments 0: everything (default).
+ *   nsc_step_phase     one quarter of nsc_step(dt) on the window: 0  N0 = N(u^n);  1  u^1 = substep(N0) -> predictor buffers;
+ *                      2  N1 = N(u^1);  3  u^{n+1} = substep(c N1 + (1 - c) N0), in place.  Outside the window the target
+ *                      arrays keep what they held.
+ *   nsc_field_pointers DEVICE pointers of the n_f arrays of a buffer set written to h_ptrs (HOST array of 4 pointers, NULL
+ *                      for T without temperature): which = 0 state (u_r, u_theta, u_z, T), 1 predictor, 2 N0, 3 N1; each
+ *                      array has the layout of a spectral field.  They stay valid until nsc_destroy; nsc_step_iterated
+ *                      and nsc_advance exchange the state pointers, so ask again after those. */
+int nsc_set_window(nsc_ctx* ctx, int j0, int nj, long long e0, long long ne);
+int nsc_step_phase(nsc_ctx* ctx, int phase, double dt);
+int nsc_field_pointers(nsc_ctx* ctx, int which, void** h_ptrs);
+
 /* Restart on another resolution ("At every restart, the spatial resolution can be
  * changed using an automated interpolation and mode padding functionality"; reading R18): the state
  * (u, T, p) of `src` is carried onto the radial grid and the mode set of `dst` and becomes the state of `dst`.

@@ -129,6 +129,8 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
     c->heated = p.Ra != 0.0;
     c->nf = c->heated ? 4 : 3;
     c->F = (size_t)c->N_r * c->M1 * c->NK;
+    c->wj1 = c->N_r;
+    c->we1 = (long long)c->M1 * c->NK;
     c->P = c->M1 * (c->K + 1);
     // radial chunk of the transform pipeline: work arrays of ~2 GiB unless told otherwise
     // default: the whole radius at once when the work arrays stay below an eighth of the device memory
@@ -318,6 +320,43 @@ static int step_body(nsc_ctx* c, double dt) {
     // N1 = N(u^1);  u^{n+1} = substep(c N1 + (1 - c) N0) from (u^n, p^n), in place
     if ((rc = launch_nonlinear(c, c->W, c->N1))) return rc;
     return launch_substep(c, c->N1, c->p.c, c->N0, 1.0 - c->p.c, dt, c->state, c->state[4]);
+}
+
+// ---- NEXT-2: the pieces of a step for a slab-decomposed run
+int nsc_set_window(nsc_ctx* c, int j0, int nj, long long e0, long long ne) {
+    if (!c) return NSC_EINVAL;
+    const long long plane = (long long)c->M1 * c->NK;
+    if (nj == 0 && ne == 0 && j0 == 0 && e0 == 0) {
+        nj = c->N_r;
+        ne = plane;
+    }
+    if (j0 < 0 || nj < 1 || j0 + nj > c->N_r || e0 < 0 || ne < 1 || e0 + ne > plane)
+        return fail(c, NSC_EINVAL, "nsc_set_window: levels [j0, j0 + nj) within [0, N_r) and modes [e0, e0 + ne) within [0, (M+1)(2K+1)), both non-empty");
+    c->wj0 = j0;
+    c->wj1 = j0 + nj;
+    c->we0 = e0;
+    c->we1 = e0 + ne;
+    c->ptr_gen += 1;                                     // a captured step graph covers the old window
+    return NSC_OK;
+}
+
+int nsc_step_phase(nsc_ctx* c, int phase, double dt) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_step_phase before nsc_set_state");
+    if (phase < 0 || phase > 3 || !(dt > 0.0)) return fail(c, NSC_EINVAL, "nsc_step_phase: phase 0..3, dt > 0");
+    switch (phase) {
+        case 0: return launch_nonlinear(c, c->state, c->N0);
+        case 1: return launch_substep(c, c->N0, 1.0, nullptr, 0.0, dt, c->W, nullptr);
+        case 2: return launch_nonlinear(c, c->W, c->N1);
+        default: return launch_substep(c, c->N1, c->p.c, c->N0, 1.0 - c->p.c, dt, c->state, c->state[4]);
+    }
+}
+
+int nsc_field_pointers(nsc_ctx* c, int which, void** h_ptrs) {
+    if (!c || !h_ptrs || which < 0 || which > 3) return NSC_EINVAL;
+    cd* const* src = which == 0 ? c->state : which == 1 ? c->W : which == 2 ? c->N0 : c->N1;
+    for (int i = 0; i < MAXF; ++i) h_ptrs[i] = i < c->nf ? (void*)src[i] : nullptr;
+    return NSC_OK;
 }
 
 static void drop_graph(nsc_ctx* c) {

@@ -91,9 +91,20 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
         if (int e = launch_dr(d, c->nf, c->stream)) return cuda_fail(c, (cudaError_t)e, "k_dr launch");
         prof_end(c);
     }
-    for (int j0 = 0; j0 < c->N_r; j0 += c->JC) {
+    const size_t rowZ = (size_t)3 * c->nf * c->Nz * c->MP;      // one radial level of zbuf
+    for (int j0 = c->wj0; j0 < c->wj1; j0 += c->JC) {
         a.j0 = j0;
-        a.nj = (c->N_r - j0 < c->JC) ? c->N_r - j0 : c->JC;
+        a.nj = (c->wj1 - j0 < c->JC) ? c->wj1 - j0 : c->JC;
+        a.zbuf = c->zbuf;
+        if (dr_after_z) {
+            // the work array holds every level at its own row; D1 at the levels of the window needs the z-transformed
+            // fields four levels beyond it on either side
+            const int h0 = j0 - NPT / 2 > 0 ? j0 - NPT / 2 : 0;
+            const int h1 = j0 + a.nj + NPT / 2 < c->N_r ? j0 + a.nj + NPT / 2 : c->N_r;
+            a.j0 = h0;
+            a.nj = h1 - h0;
+            a.zbuf = c->zbuf + (size_t)h0 * rowZ;
+        }
         a.tw = c->t.tw_z;
         prof_begin(c, NSC_K_ZINV);
         if (c->z_na) {
@@ -104,6 +115,11 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
             return cuda_fail(c, (cudaError_t)e, "k_zinv launch");
         }
         prof_end(c);
+        if (dr_after_z) {
+            a.j0 = j0;
+            a.nj = (c->wj1 - j0 < c->JC) ? c->wj1 - j0 : c->JC;
+            a.zbuf = c->zbuf + (size_t)j0 * rowZ;
+        }
         if (dr_after_z) {
             DrArgs d{};
             const size_t qstride = (size_t)c->Nz * c->MP;

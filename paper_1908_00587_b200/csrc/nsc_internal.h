@@ -96,6 +96,10 @@ struct nsc_ctx {
     int n_slices = 2;                                 // mode slices of the linear stage (NSC_LIN_SLICES overrides)
     cudaStream_t slice_stream[NSC_MAX_SLICES] = {};   // their streams
     cudaEvent_t slice_ev[NSC_MAX_SLICES + 1] = {};    // [0] fork, [1 + s] join of slice s
+    // NEXT-2 window (nsc_set_window): the nonlinear term is evaluated at the radial levels [wj0, wj1) only, the
+    // sub-step for the Fourier modes [we0, we1) only (flat index m (2K+1) + k + K); default: everything
+    int wj0 = 0, wj1 = 0;
+    long long we0 = 0, we1 = 0;
     bool have_state = false;
     std::string err;
     long long launches = 0;

@@ -23,6 +23,7 @@ EXPORTS = (
     "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_step_iterated", "nsc_nusselt", "nsc_probe", "nsc_last_error", "nsc_device_bytes",
     "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name", "nsc_graph_replays",
     "nsc_fp64_peak", "nsc_cfl_rate", "nsc_advance", "nsc_mode_coefficient", "nsc_wave_speed", "nsc_regrid",
+    "nsc_set_window", "nsc_step_phase", "nsc_field_pointers",
 )
 NSC_NKERN = 11
 
@@ -98,6 +99,9 @@ def load_library() -> C.CDLL:
     lib.nsc_mode_coefficient.argtypes = [vp, i32, i32, i32, i32, C.POINTER(dbl)]
     lib.nsc_wave_speed.argtypes = [vp, i32, i32, i32, i32, dbl, i32, C.POINTER(dbl)]
     lib.nsc_regrid.argtypes = [vp, vp]
+    lib.nsc_set_window.argtypes = [vp, i32, i32, C.c_longlong, C.c_longlong]
+    lib.nsc_step_phase.argtypes = [vp, i32, dbl]
+    lib.nsc_field_pointers.argtypes = [vp, i32, C.POINTER(vp)]
     for name in EXPORTS:
         if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count", "nsc_kernel_name",
                         "nsc_graph_replays"):
@@ -256,6 +260,26 @@ class Context:
     def regrid_from(self, src: "Context"):
         """nsc_regrid: this context's state := src's state interpolated / padded onto this resolution."""
         self._check(self._lib.nsc_regrid(self._h, src._h))
+
+    def set_window(self, j0=0, nj=0, e0=0, ne=0):
+        self._check(self._lib.nsc_set_window(self._h, j0, nj, e0, ne))
+
+    def step_phase(self, phase, dt):
+        self._check(self._lib.nsc_step_phase(self._h, phase, dt))
+
+    def field_tensors(self, which):
+        """nsc_field_pointers as torch views [N_r, (M+1)(2K+1)] (complex128, no copy) of the library's arrays:
+        which = 0 state, 1 predictor, 2 N0, 3 N1."""
+        import torch
+        ptrs = (C.c_void_p * 4)()
+        self._check(self._lib.nsc_field_pointers(self._h, which, ptrs))
+        n_modes = self.shape[1] * self.shape[2]
+        out = []
+        for i in range(self.nf):
+            iface = {"shape": (self.N_r, n_modes, 2), "typestr": "<f8", "data": (int(ptrs[i]), False), "version": 3}
+            holder = type("_DevArray", (), {"__cuda_array_interface__": iface})()
+            out.append(torch.view_as_complex(torch.as_tensor(holder, device="cuda")))
+        return out
 
     def step(self, dt):
         self._check(self._lib.nsc_step(self._h, float(dt)))

@@ -122,3 +122,49 @@ def to_mode_slab(plan: SlabPlan, x_radial, rank: int, dist=None, group=None):
         j0, j1 = plan.levels(p)
         out[j0:j1] = recvs[p]
     return out
+
+
+class SlabStepper:
+    """One rank of a slab-decomposed time step.  The rank's context has the full size; its window
+    (``nsc_set_window``) restricts the nonlinear term to the rank's radial levels and the sub-steps to its Fourier modes,
+    and after every quarter of the step (``nsc_step_phase``) the freshly written slabs are exchanged in place inside the
+    library's arrays:
+
+        phase 0  N0 = N(u^n)   at the own levels   ->  rows to columns   (N0 of the own modes at every level)
+        phase 1  u^1 = substep at the own modes    ->  columns to rows   (u^1 at the own levels + halo, every mode)
+        phase 2  N1 = N(u^1)                       ->  rows to columns
+        phase 3  u^{n+1} = substep, in place       ->  columns to rows
+
+    The pressure and its radial derivative never leave the mode-slab layout.  The context must enqueue on the stream
+    the exchanges run on (``ctx.set_stream(torch.cuda.current_stream())``)."""
+
+    BUFFER_OF_PHASE = (2, 1, 3, 0)          # nsc_field_pointers' `which` written by phase 0..3
+
+    def __init__(self, ctx, plan: SlabPlan, rank: int, dist=None, group=None):
+        self.ctx, self.plan, self.rank, self.dist, self.group = ctx, plan, rank, dist, group
+        j0, j1 = plan.levels(rank)
+        e0, e1 = plan.modes(rank)
+        ctx.set_window(j0, j1 - j0, e0, e1 - e0)
+
+    def run_phase(self, phase: int, dt: float):
+        self.ctx.step_phase(phase, dt)
+
+    def written(self, phase: int):
+        """Views of the arrays phase ``phase`` wrote (state arrays are re-read: their pointers may have been swapped)."""
+        return self.ctx.field_tensors(self.BUFFER_OF_PHASE[phase])
+
+    def exchange_after(self, phase: int):
+        plan, rank = self.plan, self.rank
+        j0, j1 = plan.levels(rank)
+        h0, h1 = plan.levels_with_halo(rank)
+        e0, e1 = plan.modes(rank)
+        for f in self.written(phase):
+            if phase in (0, 2):
+                f[:, e0:e1] = to_mode_slab(plan, f[j0:j1], rank, self.dist, self.group)
+            else:
+                f[h0:h1] = to_radial_slab(plan, f[:, e0:e1], rank, self.dist, self.group)
+
+    def step(self, dt: float):
+        for phase in range(4):
+            self.run_phase(phase, dt)
+            self.exchange_after(phase)

@@ -695,3 +695,88 @@ def test_regrid_matches_oracle(torch_cuda, src, dst):
         b.step(cb["dt"])
         nxt = b.state_to_host()
     check_parity(nxt[:nfb], ob.step(ref, cb["dt"])[:nfb], TOL_STEP, cb["K"], "one step after the regrid")
+
+
+@pytest.mark.parametrize("ci,N_r,M,K,world", [(0, 24, 8, 8, 3), (2, 16, 4, 16, 2), (3, 16, 256, 8, 2), (2, 12, 128, 128, 2)])
+def test_slab_decomposed_step_equals_the_single_context_step(torch_cuda, ci, N_r, M, K, world):
+    """NEXT-2 on one GPU: `world` contexts play the ranks of a slab-decomposed run (paper_1908_00587_b200.slabs.
+    SlabStepper: windowed phases of the step), the exchanges between them are done here by slicing (their
+    torch.distributed form is tested over gloo in tests/test_slabs_gloo.py).  Every mode of the assembled result
+    equals the plain nsc_step of one context bit for bit: levels and modes are independent."""
+    from paper_1908_00587_b200.slabs import SlabPlan, SlabStepper
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    nf = nf_of(cfg)
+    dt = cfg["dt"]
+    n_modes = (M + 1) * (2 * K + 1)
+    plan = SlabPlan(N_r=N_r, n_modes=n_modes, world=world)
+    nsteps = 3
+    with _ctx(cfg) as one:
+        st = synth.make_state(cfg, one.grid())
+        one.set_state(*_dev(torch, st))
+        for _ in range(nsteps):
+            one.step(dt)
+        ref = one.state_to_host()
+    ranks = [_ctx(cfg) for _ in range(world)]
+    try:
+        steppers = []
+        for r, c in enumerate(ranks):
+            c.set_state(*_dev(torch, st))
+            steppers.append(SlabStepper(c, plan, r))
+        for _ in range(nsteps):
+            for phase in range(4):
+                for s in steppers:
+                    s.run_phase(phase, dt)
+                torch.cuda.synchronize()
+                bufs = [s.written(phase) for s in steppers]
+                for dst in range(world):
+                    e0, e1 = plan.modes(dst)
+                    h0, h1 = plan.levels_with_halo(dst)
+                    for src in range(world):
+                        if src == dst:
+                            continue
+                        p0, p1 = plan.modes(src)
+                        j0, j1 = plan.levels(src)
+                        for f in range(nf):
+                            if phase in (0, 2):       # rows of src -> columns of dst
+                                bufs[dst][f][j0:j1, e0:e1] = bufs[src][f][j0:j1, e0:e1]
+                            else:                     # columns of src -> rows (+ halo) of dst
+                                bufs[dst][f][h0:h1, p0:p1] = bufs[src][f][h0:h1, p0:p1]
+                torch.cuda.synchronize()
+        shape = ref[0].shape
+        for r, c in enumerate(ranks):
+            e0, e1 = plan.modes(r)
+            got = c.state_to_host()
+            for i in list(range(nf)) + [4]:
+                a = got[i].reshape(N_r, -1)[:, e0:e1]
+                b = ref[i].reshape(N_r, -1)[:, e0:e1]
+                assert np.isfinite(a).all()
+                np.testing.assert_array_equal(a, b)
+        assert shape == (N_r, M + 1, 2 * K + 1)
+        # a window can be lifted again
+        ranks[0].set_window()
+        with pytest.raises(Exception):
+            ranks[0].set_window(0, N_r + 1, 0, 1)
+    finally:
+        for c in ranks:
+            c.destroy()
+
+
+def test_slab_stepper_with_one_rank_is_the_plain_step(torch_cuda):
+    """SlabStepper.step (phases + in-place exchanges through paper_1908_00587_b200.slabs) with a single rank."""
+    from paper_1908_00587_b200.slabs import SlabPlan, SlabStepper
+    torch = torch_cuda
+    cfg = synth.scaled_config(2, N_r=18, M=8, K=8)
+    res = []
+    for slab in (False, True):
+        with _ctx(cfg) as ctx:
+            ctx.set_stream(torch.cuda.current_stream())
+            st = synth.make_state(cfg, ctx.grid())
+            ctx.set_state(*_dev(torch, st))
+            stepper = SlabStepper(ctx, SlabPlan(N_r=18, n_modes=9 * 17, world=1), 0) if slab else None
+            for _ in range(2):
+                stepper.step(cfg["dt"]) if slab else ctx.step(cfg["dt"])
+            res.append(ctx.state_to_host())
+    for a, b in zip(*res):
+        if a is not None:
+            np.testing.assert_array_equal(a, b)
