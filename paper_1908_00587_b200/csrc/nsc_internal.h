@@ -87,7 +87,7 @@ struct nsc_ctx {
     bool facT_shared = false;             // T shares the u_z factors (Pr == 1)
     double fac_dt = 0.0;                  // dt the Helmholtz factors were built for (0: none)
     bool facP_ready = false;
-    // CUDA graph of one nsc_step (NSC_GRAPH=0 disables)
+    // CUDA graph of one nsc_step (nsc_params.no_graph disables)
     bool use_graph = true;
     cudaGraphExec_t graph_exec = nullptr;
     double graph_dt = 0.0;
