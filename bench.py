@@ -377,7 +377,7 @@ def run_ours(args, cfg, rank, world, local_rank):
 
         # ---- NEXT-1: the step with three corrector passes (nsc_step_iterated, tol = 0), device-resident
         # (its first call allocates 2 n_f + 2 more fields: skipped when the device has no room for them, cfg 5)
-        it_k = it_err = ms_iter = None
+        it_k = it_err = ms_iter = controller = None
         if torch.cuda.mem_get_info()[0] > (2 * nf + 3) * F:
             evi0, evi1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             ctx.step_iterated(dt, 0.0, 3)
@@ -388,6 +388,16 @@ def run_ours(args, cfg, rank, world, local_rank):
             evi1.record(stream)
             torch.cuda.synchronize()
             ms_iter = evi0.elapsed_time(evi1) / 2
+
+            # ---- NEXT-1: the step-size controller (nsc_advance, R17) for a few attempts from the same state
+            torch.cuda.synchronize()
+            tc0 = time.perf_counter()
+            adv_info, adv_log = ctx.advance(1e3 * dt, 4, dt, 1e-6, 0.5, 3)
+            torch.cuda.synchronize()
+            adv_ms = 1e3 * (time.perf_counter() - tc0)
+            controller = {"what": "nsc_advance(t_end=1000 dt, max_steps=4, dt0=dt, tol=1e-6, cfl=0.5, max_corr=3)",
+                          "attempts": [{"dt": a[0], "passes": a[1], "err": a[2], "accepted": a[3]} for a in adv_log],
+                          "cfl_rate": adv_info["cfl_rate_last"], "ms_total": adv_ms}
 
         # ---- end to end through the C ABI with HOST buffers: H2D state, step, D2H state
         ke = max(1, min(args.steps, args.e2e_steps))
@@ -504,6 +514,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         "iterated_corrector": ({"what": "nsc_step_iterated(dt, tol=0, max_corr=3): SURVEY 8(f) NEXT-1, DESIGN.md R16",
                                 "passes": it_k, "last_norm": it_err, "ms_per_step": ms_iter,
                                 "ms_per_extra_pass": (ms_iter - ms_per_step) / 2} if ms_iter is not None else None),
+        "step_size_controller": controller,
         "gpu_launches": launches,
         "clocks": clk,
         "e2e": {"value": replicas.aggregate_rate(world, 1, e2e_s), "unit": "steps/s", "h2d_bytes_per_step": nbytes_state,
