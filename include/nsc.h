@@ -101,6 +101,23 @@ int nsc_set_state_host(nsc_ctx* ctx, const void* h_ur, const void* h_uth, const 
                        const void* h_T, const void* h_p);
 int nsc_get_state_host(nsc_ctx* ctx, void* h_ur, void* h_uth, void* h_uz, void* h_T, void* h_p);
 
+/* Double-buffered host transfers for loops that feed a state in and take the result out every step (pinned HOST
+ * buffers; with pageable memory the copies are not asynchronous).  Both calls return at once.
+ *   nsc_set_state_host_async  the host buffers are copied into a staging set on a private stream -- overlapping the work
+ *                             the context's stream still does on the current state -- and the context's stream then takes
+ *                             the staging set over as the new state (device to device) and derives D1 p; calls enqueued
+ *                             afterwards see the new state.  The host buffers may be reused after nsc_host_copies_wait.
+ *   nsc_get_state_host_async  the state is snapshot on the context's stream (device to device) and the snapshot is copied
+ *                             to the host buffers on a second private stream, so that the next read-in and step overlap
+ *                             with the transfer (PCIe carries both directions at the same time).  The host buffers are
+ *                             complete after nsc_host_copies_wait.  NULL pointers are skipped.
+ * A second call of either kind waits on the device for the first one's staging set / snapshot to be free.  The first
+ * calls allocate one staging set and one snapshot of the state. */
+int nsc_set_state_host_async(nsc_ctx* ctx, const void* h_ur, const void* h_uth, const void* h_uz,
+                             const void* h_T, const void* h_p);
+int nsc_get_state_host_async(nsc_ctx* ctx, void* h_ur, void* h_uth, void* h_uz, void* h_T, void* h_p);
+int nsc_host_copies_wait(nsc_ctx* ctx);
+
 /* Steps N1-N6 of DESIGN.md (BJ (a)): N(current state), buoyancy included, written to the
  * caller's device buffers (d_NT required iff Ra != 0); the state is unchanged. */
 int nsc_nonlinear(nsc_ctx* ctx, void* d_Nr, void* d_Nth, void* d_Nz, void* d_NT);

@@ -215,6 +215,12 @@ int nsc_destroy(nsc_ctx* c) {
         if (s) cudaStreamDestroy(s);
     for (cudaEvent_t e : c->slice_ev)
         if (e) cudaEventDestroy(e);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->up_stream) cudaStreamDestroy(c->up_stream);
+    if (c->ev_uploaded) cudaEventDestroy(c->ev_uploaded);
+    if (c->ev_staged_used) cudaEventDestroy(c->ev_staged_used);
+    if (c->ev_snap) cudaEventDestroy(c->ev_snap);
+    if (c->ev_copied) cudaEventDestroy(c->ev_copied);
     cudaGetLastError();
     delete c;
     return NSC_OK;
@@ -291,6 +297,75 @@ int nsc_get_state_host(nsc_ctx* c, void* ur, void* uth, void* uz, void* T, void*
     int rc = copy_state(c, nullptr, dst, cudaMemcpyDeviceToHost, false);
     if (rc) return rc;
     NSC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NSC_OK;
+}
+
+// Double-buffered read-out: the state is snapshot on the context's stream (device to device), the snapshot leaves for
+// the host on a private stream, and the call returns; the next step and the next host-to-device copy overlap with it.
+int nsc_get_state_host_async(nsc_ctx* c, void* ur, void* uth, void* uz, void* T, void* p) {
+    if (!c) return NSC_EINVAL;
+    if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_get_state_host_async before nsc_set_state");
+    void* dst[5] = {ur, uth, uz, T, p};
+    int rc;
+    if (!c->copy_stream) {
+        for (int i = 0; i < 5; ++i)
+            if ((i != 3 || c->heated) && (rc = dev_alloc(c, &c->snap[i], c->F, false))) return rc;
+        NSC_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        NSC_CUDA(c, cudaEventCreateWithFlags(&c->ev_snap, cudaEventDisableTiming));
+        NSC_CUDA(c, cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming));
+        NSC_CUDA(c, cudaEventRecord(c->ev_copied, c->copy_stream));
+    }
+    const size_t bytes = c->F * sizeof(cd);
+    NSC_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied, 0));        // the previous snapshot has left
+    for (int i = 0; i < 5; ++i)
+        if (dst[i] && c->snap[i]) NSC_CUDA(c, cudaMemcpyAsync(c->snap[i], c->state[i], bytes, cudaMemcpyDeviceToDevice, c->stream));
+    NSC_CUDA(c, cudaEventRecord(c->ev_snap, c->stream));
+    NSC_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_snap, 0));
+    for (int i = 0; i < 5; ++i)
+        if (dst[i] && c->snap[i]) NSC_CUDA(c, cudaMemcpyAsync(dst[i], c->snap[i], bytes, cudaMemcpyDeviceToHost, c->copy_stream));
+    NSC_CUDA(c, cudaEventRecord(c->ev_copied, c->copy_stream));
+    return NSC_OK;
+}
+
+// Double-buffered read-in: the host buffers are copied into a staging set on a private stream (overlapping whatever
+// the context's stream is doing with the current state), then the context's stream takes the staging set over as the
+// new state (device to device) and derives D1 p.
+int nsc_set_state_host_async(nsc_ctx* c, const void* ur, const void* uth, const void* uz, const void* T, const void* p) {
+    if (!c) return NSC_EINVAL;
+    const void* src[5] = {ur, uth, uz, T, p};
+    for (int i = 0; i < 3 + (c->heated ? 1 : 0); ++i)
+        if (!src[i]) return fail(c, NSC_EINVAL, "nsc_set_state_host_async: required field pointer is NULL");
+    int rc;
+    if (!c->up_stream) {
+        for (int i = 0; i < 5; ++i)
+            if ((i != 3 || c->heated) && (rc = dev_alloc(c, &c->stage_in[i], c->F, false))) return rc;
+        NSC_CUDA(c, cudaStreamCreateWithFlags(&c->up_stream, cudaStreamNonBlocking));
+        NSC_CUDA(c, cudaEventCreateWithFlags(&c->ev_uploaded, cudaEventDisableTiming));
+        NSC_CUDA(c, cudaEventCreateWithFlags(&c->ev_staged_used, cudaEventDisableTiming));
+        NSC_CUDA(c, cudaEventRecord(c->ev_staged_used, c->stream));
+    }
+    const size_t bytes = c->F * sizeof(cd);
+    NSC_CUDA(c, cudaStreamWaitEvent(c->up_stream, c->ev_staged_used, 0));     // the previous staging set has been taken over
+    for (int i = 0; i < 5; ++i) {
+        if (i == 3 && !c->heated) continue;
+        if (src[i])
+            NSC_CUDA(c, cudaMemcpyAsync(c->stage_in[i], src[i], bytes, cudaMemcpyHostToDevice, c->up_stream));
+        else
+            NSC_CUDA(c, cudaMemsetAsync(c->stage_in[i], 0, bytes, c->up_stream));  // p = 0
+    }
+    NSC_CUDA(c, cudaEventRecord(c->ev_uploaded, c->up_stream));
+    NSC_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_uploaded, 0));
+    for (int i = 0; i < 5; ++i)
+        if (i != 3 || c->heated)
+            NSC_CUDA(c, cudaMemcpyAsync(c->state[i], c->stage_in[i], bytes, cudaMemcpyDeviceToDevice, c->stream));
+    NSC_CUDA(c, cudaEventRecord(c->ev_staged_used, c->stream));
+    return after_set_state(c);
+}
+
+int nsc_host_copies_wait(nsc_ctx* c) {
+    if (!c) return NSC_EINVAL;
+    if (c->up_stream) NSC_CUDA(c, cudaStreamSynchronize(c->up_stream));
+    if (c->copy_stream) NSC_CUDA(c, cudaStreamSynchronize(c->copy_stream));
     return NSC_OK;
 }
 

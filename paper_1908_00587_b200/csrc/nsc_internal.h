@@ -100,6 +100,14 @@ struct nsc_ctx {
     // sub-step for the Fourier modes [we0, we1) only (flat index m (2K+1) + k + K); default: everything
     int wj0 = 0, wj1 = 0;
     long long we0 = 0, we1 = 0;
+    // asynchronous device-to-host copies of the state (nsc_get_state_host_async): snapshot + private copy stream
+    nsc::cd* snap[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_snap = nullptr, ev_copied = nullptr;
+    // asynchronous host-to-device copies (nsc_set_state_host_async): staging set + private upload stream
+    nsc::cd* stage_in[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    cudaStream_t up_stream = nullptr;
+    cudaEvent_t ev_uploaded = nullptr, ev_staged_used = nullptr;
     bool have_state = false;
     std::string err;
     long long launches = 0;

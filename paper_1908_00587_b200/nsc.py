@@ -23,7 +23,8 @@ EXPORTS = (
     "nsc_nonlinear", "nsc_substep", "nsc_step", "nsc_step_iterated", "nsc_nusselt", "nsc_probe", "nsc_last_error", "nsc_device_bytes",
     "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name", "nsc_graph_replays",
     "nsc_fp64_peak", "nsc_cfl_rate", "nsc_advance", "nsc_mode_coefficient", "nsc_wave_speed", "nsc_regrid",
-    "nsc_set_window", "nsc_step_phase", "nsc_field_pointers",
+    "nsc_set_window", "nsc_step_phase", "nsc_field_pointers", "nsc_get_state_host_async", "nsc_host_copies_wait",
+    "nsc_set_state_host_async",
 )
 NSC_NKERN = 11
 
@@ -99,6 +100,9 @@ def load_library() -> C.CDLL:
     lib.nsc_mode_coefficient.argtypes = [vp, i32, i32, i32, i32, C.POINTER(dbl)]
     lib.nsc_wave_speed.argtypes = [vp, i32, i32, i32, i32, dbl, i32, C.POINTER(dbl)]
     lib.nsc_regrid.argtypes = [vp, vp]
+    lib.nsc_get_state_host_async.argtypes = [vp] + [vp] * 5
+    lib.nsc_set_state_host_async.argtypes = [vp] + [vp] * 5
+    lib.nsc_host_copies_wait.argtypes = [vp]
     lib.nsc_set_window.argtypes = [vp, i32, i32, C.c_longlong, C.c_longlong]
     lib.nsc_step_phase.argtypes = [vp, i32, dbl]
     lib.nsc_field_pointers.argtypes = [vp, i32, C.POINTER(vp)]
@@ -208,6 +212,20 @@ class Context:
         host = any(isinstance(a, np.ndarray) for a in (ur, uth, uz, T, p))
         fn = self._lib.nsc_get_state_host if host else self._lib.nsc_get_state
         self._check(fn(self._h, _ptr(ur), _ptr(uth), _ptr(uz), _ptr(T), _ptr(p)))
+
+    def set_state_host_async(self, ur, uth, uz, T=None, p=None):
+        """nsc_set_state_host_async from (pinned) numpy arrays; they may be reused after host_copies_wait()."""
+        self._check(self._lib.nsc_set_state_host_async(self._h, _ptr(ur), _ptr(uth), _ptr(uz), _ptr(T), _ptr(p)))
+
+    def get_state_host_async(self, ur=None, uth=None, uz=None, T=None, p=None):
+        """nsc_get_state_host_async into (pinned) numpy arrays; complete after host_copies_wait()."""
+        for a in (ur, uth, uz, T, p):
+            if a is not None and not isinstance(a, np.ndarray):
+                raise ValueError("get_state_host_async takes host (numpy) buffers")
+        self._check(self._lib.nsc_get_state_host_async(self._h, _ptr(ur), _ptr(uth), _ptr(uz), _ptr(T), _ptr(p)))
+
+    def host_copies_wait(self):
+        self._check(self._lib.nsc_host_copies_wait(self._h))
 
     def nonlinear(self, Nr, Nth, Nz, NT=None):
         self._check(self._lib.nsc_nonlinear(self._h, _ptr(Nr), _ptr(Nth), _ptr(Nz), _ptr(NT)))

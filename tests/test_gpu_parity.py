@@ -780,3 +780,43 @@ def test_slab_stepper_with_one_rank_is_the_plain_step(torch_cuda):
     for a, b in zip(*res):
         if a is not None:
             np.testing.assert_array_equal(a, b)
+
+
+def test_double_buffered_host_transfers_equal_the_synchronous_ones(torch_cuda):
+    """nsc_set_state_host_async + nsc_get_state_host_async + nsc_host_copies_wait: three rounds of (state in from the host, step, state out) with
+    the read-out of round k overlapping round k + 1; every round's host buffers hold what the synchronous call gives."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(2, N_r=20, M=16, K=16)
+    with _ctx(cfg) as ctx:
+        states = []
+        for seed in range(3):
+            st = synth.make_state(dict(cfg, seed=cfg["seed"] + seed), ctx.grid())
+            states.append(st)
+        sync_out, async_out = [], []
+        for st in states:
+            ctx.set_state(*st)
+            ctx.step(cfg["dt"])
+            sync_out.append(ctx.state_to_host())
+        pinned = [[torch.empty(st[0].shape, dtype=torch.complex128, pin_memory=True).numpy() for _ in range(5)] for _ in states]
+        pin_in = []
+        for st in states:
+            row = []
+            for a in st:
+                if a is None:
+                    row.append(None)
+                else:
+                    t = torch.empty(a.shape, dtype=torch.complex128, pin_memory=True).numpy()
+                    t[...] = a
+                    row.append(t)
+            pin_in.append(row)
+        for k, (st, out) in enumerate(zip(pin_in, pinned)):
+            if k % 2 == 0:
+                ctx.set_state_host_async(*st)       # read-in through the staging set
+            else:
+                ctx.set_state(*st)                  # ... mixed with the synchronous call
+            ctx.step(cfg["dt"])
+            ctx.get_state_host_async(*out)
+        ctx.host_copies_wait()
+        for ref, out in zip(sync_out, pinned):
+            for a, b in zip(ref, out):
+                np.testing.assert_array_equal(a, b)
