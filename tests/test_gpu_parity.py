@@ -251,10 +251,12 @@ def test_twenty_steps_at_full_cfg4(torch_cuda):
     _twenty_steps_full(torch_cuda, 3, side_stream=True)
 
 
-@pytest.mark.skipif(not os.environ.get("NSC_TEST_CFG5_STEPS"), reason="opt-in: ~6 min of oracle time and ~150 GB of host memory per step at cfg 5")
+@pytest.mark.skipif(not os.environ.get("NSC_TEST_CFG5_STEPS"), reason="opt-in: the oracle needs > 200 GB of host memory for a full step at cfg 5")
 def test_steps_at_full_cfg5(torch_cuda):
     """BASELINE.json configs[4] (N_r = 512, 513 x 1025 modes, heated; the warp-pair kernels in several radial chunks):
-    NSC_TEST_CFG5_STEPS full steps against the oracle.  Opt-in; the last recorded figures are in DESIGN.md section 9."""
+    NSC_TEST_CFG5_STEPS full steps against the oracle.  Opt-in and so far never completed: on the 196 GB host of the
+    round-2 box the oracle's step was killed for lack of memory, so full steps at cfg 5 remain unpinned (DESIGN.md
+    section 9); the nonlinear term and the sub-step are checked there on samples."""
     _twenty_steps_full(torch_cuda, 4, side_stream=True, nsteps=int(os.environ["NSC_TEST_CFG5_STEPS"]))
 
 
