@@ -325,153 +325,7 @@ __global__ void __launch_bounds__(P3_THREADS, 1) k_theta3(Nl2Args A) {
                 stage(line + lstride, 0);
             s2p_pair<+1>(x, buf, pbuf, tw, twc, tau, h, pair);
             sc_fence(sc);
-            // physical-space stage (N4): slots 0 U_r, 1 U_theta / r, 2 U_z, 3 parked line
-            if (t == 0) {
-                if constexpr (CFL) {
-                    double m0 = 0.0, m1 = 0.0;
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) {
-                        m0 = fmax(m0, fabs(x[e].x));
-                        m1 = fmax(m1, fabs(x[e].y));
-                    }
-                    line_atomic_max<32>(a.cfl + 3 * (a.j0 + jl), m0, tau);
-                    line_atomic_max<32>(a.cfl + 3 * (a.j0 + jl) + 1, m1, tau);
-                }
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    double t0[8], t1[8];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        t0[i] = x[8 * c + i].x;
-                        t1[i] = x[8 * c + i].y * ri;
-                    }
-                    sc_st8(sc, 0, c, t0);
-                    sc_st8(sc, 1, c, t1);
-                }
-            } else if (t == 1) {                               // acc = U_r d_r u_r
-                if constexpr (CFL) {
-                    double m2 = 0.0;
-#pragma unroll
-                    for (int e = 0; e < 32; ++e) m2 = fmax(m2, fabs(x[e].x));
-                    line_atomic_max<32>(a.cfl + 3 * (a.j0 + jl) + 2, m2, tau);
-                }
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    double t0[8], t2[8];
-                    Raw8 q0;
-                    sc_ld8_raw(sc, 0, c, q0);
-                    sc_wait_ld(sc);
-                    sc_unpack8(q0, t0);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        t2[i] = x[8 * c + i].x;
-                        acc[8 * c + i] = t0[i] * x[8 * c + i].y;
-                    }
-                    sc_st8(sc, 2, c, t2);
-                }
-            } else if (t == 2) {                               // N_r = -(u.grad u_r - u_theta^2 / r) -> slot 3
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    double t0[8], t1[8], t2[8];
-                    Raw8 q0;
-                    Raw8 q1;
-                    sc_ld8_raw(sc, 1, c, q0);
-                    sc_ld8_raw(sc, 2, c, q1);
-                    sc_wait_ld(sc);
-                    sc_unpack8(q0, t1);
-                    sc_unpack8(q1, t2);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        double s = fma(t1[i], x[8 * c + i].x, acc[8 * c + i]);
-                        s = fma(t2[i], x[8 * c + i].y, s);
-                        s = fma(-(t1[i] * rj), t1[i], s);
-                        t0[i] = -s;
-                    }
-                    sc_st8(sc, 3, c, t0);
-                }
-            } else if (t == 3 || t == 6) {                     // acc = U_r d_r f + (U_th / r) d_th f,  f = u_th or T
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    double t0[8], t1[8];
-                    Raw8 q0;
-                    Raw8 q1;
-                    sc_ld8_raw(sc, 0, c, q0);
-                    sc_ld8_raw(sc, 1, c, q1);
-                    sc_wait_ld(sc);
-                    sc_unpack8(q0, t0);
-                    sc_unpack8(q1, t1);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) acc[8 * c + i] = fma(t1[i], x[8 * c + i].y, t0[i] * x[8 * c + i].x);
-                }
-            } else if (t == 4) {                               // N_theta; x <- (N_r, N_theta); slot 3 <- U_r d_r u_z
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    double t0[8], t1[8], t2[8], t3[8];
-                    Raw8 q0;
-                    Raw8 q1;
-                    Raw8 q2;
-                    Raw8 q3;
-                    sc_ld8_raw(sc, 0, c, q0);
-                    sc_ld8_raw(sc, 1, c, q1);
-                    sc_ld8_raw(sc, 2, c, q2);
-                    sc_ld8_raw(sc, 3, c, q3);
-                    sc_wait_ld(sc);
-                    sc_unpack8(q0, t0);
-                    sc_unpack8(q1, t1);
-                    sc_unpack8(q2, t2);
-                    sc_unpack8(q3, t3);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        double s = fma(t2[i], x[8 * c + i].x, acc[8 * c + i]);
-                        s = fma(t0[i], t1[i], s);
-                        t2[i] = t0[i] * x[8 * c + i].y;
-                        x[8 * c + i] = mk(t3[i], -s);
-                    }
-                    sc_st8(sc, 3, c, t2);
-                }
-            } else if (t == 5) {                               // N_z = -(u.grad u_z)  (buoyancy: k_zfwd)
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    double t0[8], t1[8], t2[8];
-                    Raw8 q0;
-                    Raw8 q1;
-                    Raw8 q2;
-                    sc_ld8_raw(sc, 1, c, q0);
-                    sc_ld8_raw(sc, 2, c, q1);
-                    sc_ld8_raw(sc, 3, c, q2);
-                    sc_wait_ld(sc);
-                    sc_unpack8(q0, t1);
-                    sc_unpack8(q1, t2);
-                    sc_unpack8(q2, t0);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        double s = fma(t1[i], x[8 * c + i].x, t0[i]);
-                        s = fma(t2[i], x[8 * c + i].y, s);
-                        if (NF == 3)
-                            x[8 * c + i] = mk(-s, 0.0);
-                        else
-                            t0[i] = -s;
-                    }
-                    if (NF == 4) sc_st8(sc, 3, c, t0);         // N_z parked until N_T is known
-                }
-            } else {                                           // t == 7: N_T = -(u.grad T); x <- (N_z, N_T)
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    double t2[8], t3[8];
-                    Raw8 q2;
-                    Raw8 q3;
-                    sc_ld8_raw(sc, 2, c, q2);
-                    sc_ld8_raw(sc, 3, c, q3);
-                    sc_wait_ld(sc);
-                    sc_unpack8(q2, t2);
-                    sc_unpack8(q3, t3);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const double s = fma(t2[i], x[8 * c + i].x, acc[8 * c + i]);
-                        x[8 * c + i] = mk(t3[i], -s);
-                    }
-                }
-            }
+            theta_products<NF, CFL>(t, x, acc, sc, ri, rj, a.cfl + 3 * (a.j0 + jl), tau);
             if (t == 4 || t == NT - 1) {                       // N5: forward transform, truncation m <= M
                 p2s_pair<-1>(x, buf, pbuf, tw, twc, tau, h, pair);
                 cd* O = a.tbuf + (size_t)(t == 4 ? 0 : 2) * qstride + loff;
