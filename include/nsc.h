@@ -227,8 +227,46 @@ int nsc_nusselt(nsc_ctx* ctx, double* h_out);
  * 4 p.  *h_value: HOST double.  Synchronises the stream. */
 int nsc_probe(nsc_ctx* ctx, int field, int j, double theta, double z, double* h_value);
 
+/* The probe of nsc_probe without a context and without a single allocation (Fig. 3b: the
+ * probe signal is what a run is watched by).
+ *
+ * For whom: code that reads a probe from a state it holds itself but must not allocate device memory -- a
+ * per-step monitoring hook next to a solver that has filled the device on purpose (the N_r = 512 configuration
+ * holds 148 of 180 GB; a host framework's pool owns the rest, so a cudaMalloc fails or eats into it), code
+ * between a solver's kernels where the device-wide stall of cudaMalloc / cudaFree would be paid every step, or
+ * code in a region where its host program bans allocating runtime calls.  nsc_probe cannot serve them: it
+ * needs a context, and nsc_create allocates.
+ *
+ * What it does: the Fourier series of one field at radial node j, evaluated at (theta, z), written to *d_value
+ * -- the same sum as nsc_probe, added up in a fixed order (block partials, then the partials in index order),
+ * so repeated calls on the same data give the same bits.
+ *   d_field     DEVICE, caller's: one spectral field [N_r][M_theta+1][2 K_z+1] complex128 as described at the
+ *               top; only level j is read.  k_theta0, alpha: the base wavenumbers the field belongs to.
+ *   d_value     DEVICE, caller's: one double, overwritten.
+ *   cuda_stream cudaStream_t as void* (NULL: legacy default stream).  The call only enqueues (one 256-byte
+ *               memset, one kernel) and returns; *d_value is ready when that stream work has finished.
+ *   The device that owns d_field, d_value and the stream must be the calling thread's current device.
+ * Memory: nothing is allocated or freed, by this call or by anything it calls (no cudaMalloc / cudaFree, no
+ * library routine that allocates).  The block partials and the blocks' arrival counter sit in a fixed array
+ * inside the library image, NSC_PROBE_STATIC_SCRATCH_BYTES per GPU that has loaded the library, held until the
+ * process exits.
+ * Limit: M_theta <= 512 and K_z <= 512 (525 825 modes, what the array is laid out for; also nsc_create's
+ * limit).  Anything larger is refused with NSC_EINVAL and a text saying so; nothing is launched.
+ * First call on each device: looks up the array's device address (cudaGetSymbolAddress, with that device
+ * current; the result is kept) and lets the driver load the kernel.  Make that first call during start-up,
+ * before any stream capture is begun on that device.
+ * Sharing: every call on a device uses the same array.  It keeps the previous call's contents -- the call
+ * clears the counter itself, on `cuda_stream`, before the kernel -- and two calls whose device work overlaps
+ * in time (two streams without an event between them, two host threads) race on it and both results are
+ * wrong.  Keep the calls of one device on one stream or order them with events.
+ * Errors: NSC_EINVAL (NULL pointer, sizes out of range, j outside [0, N_r), k_theta0 < 1, alpha <= 0,
+ * non-finite alpha / theta / z) before any CUDA call; NSC_ECUDA if a CUDA call fails.  Text: nsc_last_error(NULL). */
+#define NSC_PROBE_STATIC_SCRATCH_BYTES 4608
+int nsc_probe_static(const void* d_field, int N_r, int M_theta, int K_z, int k_theta0, double alpha, int j,
+                     double theta, double z, double* d_value, void* cuda_stream);
+
 /* Text of the last error of this context ("" if none); valid until the next call on ctx.
- * With ctx == NULL: the text of the last failed nsc_create on this thread. */
+ * With ctx == NULL: the text of the last failed nsc_create or nsc_probe_static on this thread. */
 const char* nsc_last_error(const nsc_ctx* ctx);
 
 /* Bytes of device memory the context holds (state + work + factors), for reports. */

@@ -32,7 +32,8 @@ def _nvcc() -> str:
 def _sources():
     units = [("plan", "plan.cu", []), ("api", "api.cu", []), ("linear", "linear.cu", []),
              ("nonlinear", "nonlinear.cu", []), ("nonlinear_v2", "nonlinear_v2.cu", []),
-             ("peaks", "peaks.cu", []), ("regrid", "regrid.cu", [])]
+             ("peaks", "peaks.cu", []), ("regrid", "regrid.cu", []),
+             ("probe_static", "probe_static.cu", [])]
     units += [(f"nonlinear_inst_{n}", "nonlinear_inst.cu", [f"-DNSC_FFT_N={n}"]) for n in FFT_LENGTHS]
     return units
 

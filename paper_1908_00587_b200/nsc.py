@@ -24,7 +24,7 @@ EXPORTS = (
     "nsc_launch_count", "nsc_set_profiling", "nsc_profile_read", "nsc_kernel_name", "nsc_graph_replays",
     "nsc_fp64_peak", "nsc_cfl_rate", "nsc_advance", "nsc_mode_coefficient", "nsc_wave_speed", "nsc_regrid",
     "nsc_set_window", "nsc_step_phase", "nsc_field_pointers", "nsc_get_state_host_async", "nsc_host_copies_wait",
-    "nsc_set_state_host_async",
+    "nsc_set_state_host_async", "nsc_probe_static",
 )
 NSC_NKERN = 11
 
@@ -106,6 +106,7 @@ def load_library() -> C.CDLL:
     lib.nsc_set_window.argtypes = [vp, i32, i32, C.c_longlong, C.c_longlong]
     lib.nsc_step_phase.argtypes = [vp, i32, dbl]
     lib.nsc_field_pointers.argtypes = [vp, i32, C.POINTER(vp)]
+    lib.nsc_probe_static.argtypes = [vp, i32, i32, i32, i32, dbl, i32, dbl, dbl, vp, vp]
     for name in EXPORTS:
         if name not in ("nsc_last_error", "nsc_device_bytes", "nsc_launch_count", "nsc_kernel_name",
                         "nsc_graph_replays"):
@@ -136,6 +137,29 @@ def fp64_peak(kind: int = 0, device: int = -1) -> float:
     if rc != NSC_OK:
         raise NscError(rc, "nsc_fp64_peak failed (no CUDA device?)")
     return v.value
+
+
+def probe_static(field, k_theta0, alpha, j, theta, z, out, stream=None):
+    """nsc_probe_static: the value at (r_j, theta, z) of the physical field whose spectral coefficients ``field`` holds
+    (a contiguous complex128 CUDA tensor [N_r, M_theta+1, 2 K_z+1] of the caller's), written to ``out`` (a float64 CUDA
+    tensor with one element, also the caller's) by work enqueued on ``stream`` (a torch.cuda.Stream; None: torch's
+    current stream).  For callers that must not allocate device memory: no context is needed and the library
+    allocates nothing -- see include/nsc.h for the size limit (M_theta, K_z <= 512), the first-call set-up and why
+    calls that overlap on one GPU must be ordered.  Returns at once; ``out`` is valid once the stream has run."""
+    import torch
+    lib = load_library()
+    if field.dtype != torch.complex128 or not field.is_contiguous() or field.dim() != 3 or not field.is_cuda:
+        raise ValueError("field must be a contiguous complex128 CUDA tensor [N_r, M_theta+1, 2 K_z+1]")
+    if out.dtype != torch.float64 or out.numel() != 1 or not out.is_cuda:
+        raise ValueError("out must be a float64 CUDA tensor with one element")
+    N_r, M1, NK = field.shape
+    if NK % 2 != 1:
+        raise ValueError("the last axis of field holds 2 K_z + 1 axial modes: an odd number")
+    s = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib.nsc_probe_static(C.c_void_p(field.data_ptr()), N_r, M1 - 1, (NK - 1) // 2, int(k_theta0), float(alpha),
+                              int(j), float(theta), float(z), C.c_void_p(out.data_ptr()), C.c_void_p(s.cuda_stream))
+    if rc != NSC_OK:
+        raise NscError(rc, lib.nsc_last_error(None).decode())
 
 
 class Context:
