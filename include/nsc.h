@@ -189,8 +189,10 @@ int nsc_wave_speed(nsc_ctx* ctx, int field, int j, int m, int k, double dt, int 
  * independent in the linear terms, radial levels in the nonlinear terms).  Every rank holds a
  * context of the full size and computes only its window; the Python module paper_1908_00587_b200.slabs moves the slabs
  * between the ranks (torch.distributed) directly inside the library's arrays.
- *   nsc_set_window     nsc_nonlinear / phases 0, 2 evaluate the radial levels [j0, j0 + nj) only (they read the fields at
- *                      those levels and four beyond on either side); nsc_substep / phases 1, 3 treat the Fourier modes
+ *   nsc_set_window     nsc_nonlinear / phases 0, 2 evaluate the radial levels [j0, j0 + nj) only.  They read the fields at
+ *                      the levels the nine-point stencils of the window reach, [s(j0), s(j0 + nj - 1) + 9) with
+ *                      s(j) = clamp(j - 4, 0, N_r - 9): four levels beyond the window on either side, and the nine levels
+ *                      next to a wall however short the window.  nsc_substep / phases 1, 3 treat the Fourier modes
  *                      [e0, e0 + ne) only (flat index m (2 K_z + 1) + k + K_z).  All four arguments 0: everything (default).
  *   nsc_step_phase     one quarter of nsc_step(dt) on the window: 0  N0 = N(u^n);  1  u^1 = substep(N0) -> predictor buffers;
  *                      2  N1 = N(u^1);  3  u^{n+1} = substep(c N1 + (1 - c) N0), in place.  Outside the window the target

@@ -97,10 +97,12 @@ int launch_nonlinear(nsc_ctx* c, cd* const* f, cd* const* out) {
         a.nj = (c->wj1 - j0 < c->JC) ? c->wj1 - j0 : c->JC;
         a.zbuf = c->zbuf;
         if (dr_after_z) {
-            // the work array holds every level at its own row; D1 at the levels of the window needs the z-transformed
-            // fields four levels beyond it on either side
-            const int h0 = j0 - NPT / 2 > 0 ? j0 - NPT / 2 : 0;
-            const int h1 = j0 + a.nj + NPT / 2 < c->N_r ? j0 + a.nj + NPT / 2 : c->N_r;
+            // the work array holds every level at its own row; D1 at level j reads the z-transformed fields at the
+            // nine rows s0(j) .. s0(j) + 8 with s0(j) = clamp(j - 4, 0, N_r - 9): four levels beyond the window on
+            // either side, and all nine rows next to a wall even when the window is shorter than five levels
+            const int smax = c->N_r - NPT, jl = j0 + a.nj - 1;
+            const int h0 = j0 - NPT / 2 < 0 ? 0 : (j0 - NPT / 2 > smax ? smax : j0 - NPT / 2);
+            const int h1 = (jl - NPT / 2 < 0 ? 0 : (jl - NPT / 2 > smax ? smax : jl - NPT / 2)) + NPT;
             a.j0 = h0;
             a.nj = h1 - h0;
             a.zbuf = c->zbuf + (size_t)h0 * rowZ;

@@ -12,8 +12,8 @@ Layouts of one spectral field with n_modes = (M + 1)(2 K + 1) coefficients per r
 
   mode slab    [N_r, e1 - e0]              all radial levels of the modes e0 .. e1 - 1 of this rank   (linear stage)
   radial slab  [h1 - h0, n_modes]          all modes of the levels h0 .. h1 - 1 = the rank's own levels j0 .. j1 - 1
-                                           plus ``halo`` levels on either side (the nine-point radial stencil of N1
-                                           needs four)                                                  (nonlinear stage)
+                                           plus the levels their nine-point radial stencils of N1 reach: four on
+                                           either side, all nine next to a wall                        (nonlinear stage)
 """
 from __future__ import annotations
 
@@ -32,6 +32,8 @@ class SlabPlan:
             raise ValueError("the number of ranks must divide N_r (PAPER.md:72)")
         if self.n_modes < self.world:
             raise ValueError("fewer Fourier modes than ranks")
+        if self.N_r < 2 * self.halo + 1:
+            raise ValueError("fewer radial levels than one stencil")
 
     # ---- ownership
     def levels(self, rank: int) -> tuple[int, int]:
@@ -40,9 +42,14 @@ class SlabPlan:
         return rank * n, (rank + 1) * n
 
     def levels_with_halo(self, rank: int) -> tuple[int, int]:
-        """The levels ``rank`` needs as input of the nonlinear stage: its own plus the stencil halo, clipped."""
+        """The levels ``rank`` needs as input of the nonlinear stage: the union of the radial stencils of its own
+        levels.  The stencil of level j is the 2 halo + 1 levels starting at clamp(j - halo, 0, N_r - 2 halo - 1): halo
+        levels on either side in the interior, one-sided next to a wall -- so a slab of fewer than halo + 1 levels at a
+        wall still needs the first (last) 2 halo + 1 levels."""
         j0, j1 = self.levels(rank)
-        return max(0, j0 - self.halo), min(self.N_r, j1 + self.halo)
+        width = 2 * self.halo + 1
+        start = lambda j: min(max(j - self.halo, 0), self.N_r - width)
+        return start(j0), start(j1 - 1) + width
 
     def modes(self, rank: int) -> tuple[int, int]:
         """Fourier modes [e0, e1) (flat index m (2K+1) + k + K) whose sub-step ``rank`` computes; the first

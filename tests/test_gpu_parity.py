@@ -706,7 +706,41 @@ def test_regrid_matches_oracle(torch_cuda, src, dst):
     check_parity(nxt[:nfb], ob.step(ref, cb["dt"])[:nfb], TOL_STEP, cb["K"], "one step after the regrid")
 
 
-@pytest.mark.parametrize("ci,N_r,M,K,world", [(0, 24, 8, 8, 3), (2, 16, 4, 16, 2), (3, 16, 256, 8, 2), (2, 12, 128, 128, 2)])
+@pytest.mark.parametrize("ci,N_r,M,K", [(2, 12, 128, 128), (0, 14, 8, 8), (3, 11, 256, 8)])
+def test_nonlinear_window_shorter_than_the_stencil_at_either_wall(torch_cuda, ci, N_r, M, K):
+    """nsc_set_window with one or two levels at j0 = 0 and at the outer wall: the nine-point stencil there is
+    one-sided (s0 = clamp(j - 4, 0, N_r - 9)), so the window reads nine levels, not its own plus four.  Before every
+    windowed evaluation the work arrays are filled by an evaluation of another state, so a level the windowed
+    pass forgets to transform shows up as a wrong result.  (2, 12, 128, 128) runs the single-chunk warp kernels
+    (D1 applied inside the work array), (0, 14, 8, 8) the generic ones, (3, 11, 256, 8) a mix."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(ci, N_r=N_r, M=M, K=K)
+    nf = nf_of(cfg)
+    n_modes = (M + 1) * (2 * K + 1)
+    with _ctx(cfg) as ctx:
+        st = synth.make_state(cfg, ctx.grid())
+        rng = np.random.default_rng(cfg["seed"] + 5)
+        other = [None if f is None else f + 0.5 * (rng.standard_normal(f.shape) + 1j * rng.standard_normal(f.shape))
+                 for f in st]
+        ctx.set_state(*_dev(torch, st))
+        full = ctx.nonlinear_to_host()
+        for j0, nj in [(0, 1), (N_r - 1, 1), (0, 2), (N_r - 2, 2), (3, 1), (N_r - 5, 1), (N_r // 2, 1), (2, 4)]:
+            ctx.set_window()
+            ctx.set_state(*_dev(torch, other))
+            ctx.nonlinear_to_host()                      # the work arrays now hold the other state's lines
+            ctx.set_state(*_dev(torch, st))
+            ctx.set_window(j0, nj, 0, n_modes)
+            bufs = [torch.full(ctx.shape, float("nan"), dtype=torch.complex128, device="cuda") for _ in range(nf)]
+            ctx.nonlinear(*bufs)
+            torch.cuda.synchronize()
+            for i in range(nf):
+                g = bufs[i].cpu().numpy()
+                np.testing.assert_array_equal(g[j0:j0 + nj], full[i][j0:j0 + nj], err_msg=f"window ({j0}, {nj}), field {i}")
+                assert np.isnan(g[:j0]).all() and np.isnan(g[j0 + nj:]).all(), "levels outside the window were written"
+
+
+@pytest.mark.parametrize("ci,N_r,M,K,world", [(0, 24, 8, 8, 3), (2, 16, 4, 16, 2), (3, 16, 256, 8, 2), (2, 12, 128, 128, 2),
+                                              (0, 16, 8, 8, 4), (2, 12, 128, 128, 3)])
 def test_slab_decomposed_step_equals_the_single_context_step(torch_cuda, ci, N_r, M, K, world):
     """NEXT-2 on one GPU: `world` contexts play the ranks of a slab-decomposed run (paper_1908_00587_b200.slabs.
     SlabStepper: windowed phases of the step), the exchanges between them are done here by slicing (their

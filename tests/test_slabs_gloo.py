@@ -30,6 +30,11 @@ def test_plan_partitions_levels_and_modes():
     lev = [plan.levels(r) for r in range(4)]
     assert lev == [(0, 8), (8, 16), (16, 24), (24, 32)]
     assert [plan.levels_with_halo(r) for r in range(4)] == [(0, 12), (4, 20), (12, 28), (20, 32)]
+    # slabs of four levels: the one-sided stencils next to a wall reach nine levels (s0 = clamp(j - 4, 0, N_r - 9))
+    assert [SlabPlan(N_r=16, n_modes=153, world=4).levels_with_halo(r) for r in range(4)] == [(0, 9), (0, 12), (4, 16), (7, 16)]
+    assert [SlabPlan(N_r=32, n_modes=153, world=8).levels_with_halo(r) for r in (0, 1, 6, 7)] == [(0, 9), (0, 12), (20, 32), (23, 32)]
+    assert SlabPlan(N_r=16, n_modes=153, world=16).levels_with_halo(15) == (7, 16)
+    assert SlabPlan(N_r=16, n_modes=153, world=16).levels_with_halo(8) == (4, 13)
     mo = [plan.modes(r) for r in range(4)]
     assert mo[0][0] == 0 and mo[-1][1] == 153 and all(a[1] == b[0] for a, b in zip(mo, mo[1:]))
     assert sorted(e1 - e0 for e0, e1 in mo) == [38, 38, 38, 39]
