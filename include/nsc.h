@@ -212,8 +212,9 @@ int nsc_field_pointers(nsc_ctx* ctx, int which, void** h_ptrs);
  *            node (window start clamp(c - 4, 0, N_r,src - 9)); a target node that coincides with a source node takes
  *            its value exactly;
  *   modes  : coefficients of modes `src` does not hold are zero, modes `dst` does not hold are dropped.
- * Both contexts must live on the same device and agree in eta, alpha and k_theta0 (NSC_EINVAL otherwise); N_r, M_theta,
- * K_z, the grid family, Re_i, Re_o, Ra, Pr may differ.  A temperature field of `src` is dropped if `dst` has none;
+ * `dst` and `src` must be two different contexts on the same device that agree in eta, alpha and k_theta0 (NSC_EINVAL
+ * otherwise, checked before anything is touched; the call makes that device current while it runs and puts the caller's
+ * current device back); N_r, M_theta, K_z, the grid family, Re_i, Re_o, Ra, Pr may differ.  A temperature field of `src` is dropped if `dst` has none;
  * `dst` with temperature needs `src` with temperature.  `src` is unchanged.  Synchronises both streams. */
 int nsc_regrid(nsc_ctx* dst, nsc_ctx* src);
 
@@ -308,7 +309,9 @@ long long nsc_graph_replays(const nsc_ctx* ctx);
 /* Measured fp64 peak of a device: a register-only
  * kernel on every SM, timed with CUDA events, best of six runs.  kind 0: DFMA only (2 flop each);
  * kind 1: DADD and DMUL alternating (1 flop each).  device: CUDA ordinal, -1 = current.
- * *h_tflops (HOST double) receives TFLOP/s.  Synchronises the device; needs no context. */
+ * *h_tflops (HOST double) receives TFLOP/s.  Synchronises the device; needs no context.  The calling thread's
+ * current device is the same after the call as before it.  NSC_EINVAL for an ordinal the machine does not have,
+ * NSC_ECUDA if a CUDA call fails or no positive, finite rate could be measured. */
 int nsc_fp64_peak(int kind, int device, double* h_tflops);
 
 #ifdef __cplusplus

@@ -118,6 +118,7 @@ int nsc_create_ex(nsc_ctx** out, const nsc_params* pp) {
     nsc_ctx* c = new (std::nothrow) nsc_ctx();
     if (!c) return fail(nullptr, NSC_ENOMEM, "nsc_create: out of host memory");
     c->p = p;
+    cudaGetDevice(&c->dev);
     c->N_r = p.N_r;
     c->M = p.M_theta;
     c->K = p.K_z;

@@ -59,6 +59,7 @@ struct nsc_ctx {
     size_t F = 0;                         // complex elements per spectral field
     int P = 0;                            // pairs (m, |k|): (M+1)(K+1)
     cudaStream_t stream = nullptr;
+    int dev = -1;                         // ordinal of the device the context was created on
     std::vector<double> r;                // radial nodes (host copy)
     nsc::Tables t;
     nsc::cd* state[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // u_r, u_theta, u_z, T, p
@@ -146,6 +147,30 @@ int launch_probe(nsc_ctx* c, const cd* field, int j, double theta, double z, dou
 // them, and they also count the launch.
 void prof_begin(nsc_ctx* c, int kernel_id);
 void prof_end(nsc_ctx* c);
+
+// Makes `dev` the calling thread's current device for the lifetime of the guard and puts the caller's device back
+// afterwards (entry points that must run on a given device whatever is current).  ok() is false if that failed.
+class DeviceGuard {
+    int prev_ = -1;
+    bool ok_ = false;
+public:
+    explicit DeviceGuard(int dev) {
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess) return;
+        if (cur == dev) {
+            ok_ = true;
+        } else if (cudaSetDevice(dev) == cudaSuccess) {
+            ok_ = true;
+            prev_ = cur;
+        }
+    }
+    ~DeviceGuard() {
+        if (prev_ >= 0) cudaSetDevice(prev_);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+    bool ok() const { return ok_; }
+};
 
 int fail(nsc_ctx* c, int code, const std::string& msg);
 int cuda_fail(nsc_ctx* c, cudaError_t e, const char* what);

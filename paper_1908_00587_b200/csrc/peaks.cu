@@ -5,6 +5,7 @@
 //   kind 0: DFMA only (2 flop per instruction)
 //   kind 1: DADD and DMUL alternating (1 flop per instruction) -- the rate the butterflies'
 //           add/sub-heavy parts can reach
+#include <cmath>
 #include "nsc_internal.h"
 
 namespace nsc {
@@ -48,36 +49,47 @@ extern "C" int nsc_fp64_peak(int kind, int device, double* h_tflops) {
         cudaGetLastError();
         return NSC_ECUDA;
     }
-    if (device >= 0 && cudaSetDevice(device) != cudaSuccess) return NSC_ECUDA;
-    int dev = 0, sms = 0;
-    cudaGetDevice(&dev);
+    int dev = device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return NSC_ECUDA;
+    if (dev >= ndev) return NSC_EINVAL;
+    DeviceGuard on_device(dev);                  // the caller's current device is put back on every return path
+    if (!on_device.ok()) return NSC_ECUDA;
+    int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return NSC_ECUDA;
     double* sink = nullptr;
     if (cudaMalloc(&sink, sizeof(double)) != cudaSuccess) return NSC_ENOMEM;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        if (e0) cudaEventDestroy(e0);
+        cudaFree(sink);
+        return NSC_ECUDA;
+    }
     const int grid = sms * 8, outer = 2048;     // 8 CTAs of 8 warps per SM: every scheduler has 16 warps to pick from
     const double a = 0.999999999, b = 1e-9;
     double best = 0.0;
-    for (int rep = 0; rep < 6; ++rep) {          // first repetitions warm the clocks up; the best one counts
-        cudaEventRecord(e0);
+    bool failed = false;
+    for (int rep = 0; rep < 6 && !failed; ++rep) {   // first repetitions warm the clocks up; the best one counts
+        failed = cudaEventRecord(e0) != cudaSuccess;
         if (kind == 0)
             k_fp64_peak<0><<<grid, 256>>>(sink, outer, a, b);
         else
             k_fp64_peak<1><<<grid, 256>>>(sink, outer, a, b);
-        cudaEventRecord(e1);
-        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        failed = failed || cudaGetLastError() != cudaSuccess || cudaEventRecord(e1) != cudaSuccess ||
+                 cudaEventSynchronize(e1) != cudaSuccess;
         float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
+        if (failed || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) {
+            failed = true;
+            break;
+        }
+        if (!(ms > 0.f)) continue;                   // a timer reading of zero would report an infinite rate
         const double inst = (double)grid * 256.0 * outer * PK_INNER * PK_CHAINS;
-        const double tf = inst * (kind == 0 ? 2.0 : 1.0) / (ms * 1e-3) / 1e12;
-        if (tf > best) best = tf;
+        const double tf = inst * (kind == 0 ? 2.0 : 1.0) / ((double)ms * 1e-3) / 1e12;
+        if (std::isfinite(tf) && tf > best) best = tf;
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(sink);
-    if (cudaGetLastError() != cudaSuccess || best == 0.0) return NSC_ECUDA;
+    if (failed || cudaGetLastError() != cudaSuccess || !(best > 0.0) || !std::isfinite(best)) return NSC_ECUDA;
     *h_tflops = best;
     return NSC_OK;
 }

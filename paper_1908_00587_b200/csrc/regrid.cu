@@ -75,6 +75,10 @@ using namespace nsc;
 
 extern "C" int nsc_regrid(nsc_ctx* d, nsc_ctx* s) {
     if (!d || !s) return NSC_EINVAL;
+    if (d == s) return fail(d, NSC_EINVAL, "nsc_regrid: source and target must be two contexts (the kernel reads the source rows while it writes the target)");
+    if (d->dev != s->dev)
+        return fail(d, NSC_EINVAL, "nsc_regrid: the two contexts live on different devices (" + std::to_string(s->dev) + " and " +
+                                       std::to_string(d->dev) + ")");
     if (!s->have_state) return fail(d, NSC_ESTATE, "nsc_regrid: the source context has no state");
     if (d->p.eta != s->p.eta || d->p.alpha != s->p.alpha || d->p.k_theta0 != s->p.k_theta0)
         return fail(d, NSC_EINVAL, "nsc_regrid: eta, alpha and k_theta0 of the two contexts must agree (same domain, same wavenumbers)");
@@ -100,6 +104,8 @@ extern "C" int nsc_regrid(nsc_ctx* d, nsc_ctx* s) {
     }
     double* d_w = nullptr;
     int* d_s0 = nullptr;
+    DeviceGuard on_device(d->dev);                         // the tables and the launch belong to the contexts' device
+    if (!on_device.ok()) return fail(d, NSC_ECUDA, "nsc_regrid: cannot make the contexts' device current");
     NSC_CUDA(d, cudaStreamSynchronize(s->stream));         // the source state is complete
     NSC_CUDA(d, cudaMalloc(&d_w, sizeof(double) * w.size()));
     cudaError_t e = cudaMalloc(&d_s0, sizeof(int) * s0.size());

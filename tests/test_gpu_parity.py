@@ -701,6 +701,11 @@ def test_regrid_matches_oracle(torch_cuda, src, dst):
         for g, s_ in zip(a2.state_to_host(), st):
             if s_ is not None:
                 np.testing.assert_array_equal(g, s_)
+        with pytest.raises(Exception, match="two contexts"):
+            a.regrid_from(a)                         # in place: refused, the kernel would read rows it is overwriting
+        for g, s_ in zip(a.state_to_host(), st):
+            if s_ is not None:
+                np.testing.assert_array_equal(g, s_)
         b.step(cb["dt"])
         nxt = b.state_to_host()
     check_parity(nxt[:nfb], ob.step(ref, cb["dt"])[:nfb], TOL_STEP, cb["K"], "one step after the regrid")
@@ -863,3 +868,20 @@ def test_double_buffered_host_transfers_equal_the_synchronous_ones(torch_cuda):
         for ref, out in zip(sync_out, pinned):
             for a, b in zip(ref, out):
                 np.testing.assert_array_equal(a, b)
+
+
+def test_measured_fp64_peaks_are_sane_and_leave_the_current_device_alone(torch_cuda):
+    """nsc_fp64_peak (bench.py's roofline denominators): a positive finite rate below the nominal 148 SM x 64 lanes
+    x 2 flop x 2.1 GHz = 40 TFLOP/s, add/mul at about half the FMA rate, bad ordinals refused, and the calling
+    thread's current device unchanged."""
+    import ctypes as C
+    torch = torch_cuda
+    from paper_1908_00587_b200 import nsc
+    before = torch.cuda.current_device()
+    fma, addmul = nsc.fp64_peak(0, 0), nsc.fp64_peak(1, -1)
+    assert torch.cuda.current_device() == before
+    assert np.isfinite(fma) and 10.0 < fma < 40.0, fma
+    assert np.isfinite(addmul) and 0.4 * fma < addmul < 0.6 * fma, (fma, addmul)
+    lib, v = nsc.load_library(), C.c_double(-1.0)
+    assert lib.nsc_fp64_peak(0, torch.cuda.device_count(), C.byref(v)) == nsc.NSC_EINVAL
+    assert lib.nsc_fp64_peak(2, 0, C.byref(v)) == nsc.NSC_EINVAL and v.value == -1.0
