@@ -999,13 +999,14 @@ int launch_substep(nsc_ctx* c, cd* const* E0, double w0, cd* const* E1, double w
         // left for the SMs its finished columns occupied), the next sweep of the other slice fills the machine.
         // With per-kernel profiling on, one slice on the caller's stream (the event brackets need one stream).
         const int nsl = (c->profiling || !c->slice_stream[0]) ? 1 : c->n_slices;
-        const int w0 = (int)c->we0, w1 = (int)c->we1;                      // the window of modes (default: all)
-        const int per = ((w1 - w0 + nsl - 1) / nsl + 127) / 128 * 128;     // multiple of every block width
+        // the window of modes (default: all); not w0 / w1: those are this function's weights of E0 and E1
+        const int we_lo = (int)c->we0, we_hi = (int)c->we1;
+        const int per = ((we_hi - we_lo + nsl - 1) / nsl + 127) / 128 * 128;   // multiple of every block width
         if (nsl > 1) {
             NSC_CUDA(c, cudaEventRecord(c->slice_ev[0], c->stream));
         }
         for (int sl = 0; sl < nsl; ++sl) {
-            const int eb = w0 + sl * per, ee = (eb + per < w1) ? eb + per : w1;
+            const int eb = we_lo + sl * per, ee = (eb + per < we_hi) ? eb + per : we_hi;
             if (eb >= ee) continue;
             cudaStream_t st = (nsl > 1) ? c->slice_stream[sl] : c->stream;
             if (nsl > 1) NSC_CUDA(c, cudaStreamWaitEvent(st, c->slice_ev[0], 0));
