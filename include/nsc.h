@@ -110,9 +110,11 @@ int nsc_get_state_host(nsc_ctx* ctx, void* h_ur, void* h_uth, void* h_uz, void* 
  *   nsc_get_state_host_async  the state is snapshot on the context's stream (device to device) and the snapshot is copied
  *                             to the host buffers on a second private stream, so that the next read-in and step overlap
  *                             with the transfer (PCIe carries both directions at the same time).  The host buffers are
- *                             complete after nsc_host_copies_wait.  NULL pointers are skipped.
+ *                             complete after nsc_host_copies_wait.  NULL pointers are skipped; h_T on a context without
+ *                             temperature is refused (NSC_EINVAL) instead of being left unwritten without notice.
  * A second call of either kind waits on the device for the first one's staging set / snapshot to be free.  The first
- * calls allocate one staging set and one snapshot of the state. */
+ * calls allocate one staging set and one snapshot of the state and create a private stream and two events each; if that
+ * set-up fails halfway the call returns the error, keeps what exists and the next call creates only what is missing. */
 int nsc_set_state_host_async(nsc_ctx* ctx, const void* h_ur, const void* h_uth, const void* h_uz,
                              const void* h_T, const void* h_p);
 int nsc_get_state_host_async(nsc_ctx* ctx, void* h_ur, void* h_uth, void* h_uz, void* h_T, void* h_p);

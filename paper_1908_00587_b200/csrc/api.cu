@@ -301,21 +301,35 @@ int nsc_get_state_host(nsc_ctx* c, void* ur, void* uth, void* uz, void* T, void*
     return NSC_OK;
 }
 
+// First-use set-up shared by the two double-buffered transfers: one buffer set of the state's size, a private stream
+// and two events, the second of which is recorded once on `first_on` so that the first wait finds it signalled.
+// `*ready` is set last.  A call that failed halfway leaves what it created in place (owned by the context, released by
+// nsc_destroy); the next call creates only what is still missing instead of allocating everything again or running
+// with null events.
+static int transfer_setup(nsc_ctx* c, cd** bufs, cudaStream_t* priv, cudaEvent_t* ev_a, cudaEvent_t* ev_b,
+                          bool first_on_private, bool* ready) {
+    if (*ready) return NSC_OK;
+    int rc;
+    for (int i = 0; i < 5; ++i)
+        if ((i != 3 || c->heated) && !bufs[i] && (rc = dev_alloc(c, &bufs[i], c->F, false))) return rc;
+    if (!*priv) NSC_CUDA(c, cudaStreamCreateWithFlags(priv, cudaStreamNonBlocking));
+    if (!*ev_a) NSC_CUDA(c, cudaEventCreateWithFlags(ev_a, cudaEventDisableTiming));
+    if (!*ev_b) NSC_CUDA(c, cudaEventCreateWithFlags(ev_b, cudaEventDisableTiming));
+    NSC_CUDA(c, cudaEventRecord(*ev_b, first_on_private ? *priv : c->stream));
+    *ready = true;
+    return NSC_OK;
+}
+
 // Double-buffered read-out: the state is snapshot on the context's stream (device to device), the snapshot leaves for
 // the host on a private stream, and the call returns; the next step and the next host-to-device copy overlap with it.
 int nsc_get_state_host_async(nsc_ctx* c, void* ur, void* uth, void* uz, void* T, void* p) {
     if (!c) return NSC_EINVAL;
     if (!c->have_state) return fail(c, NSC_ESTATE, "nsc_get_state_host_async before nsc_set_state");
+    if (T && !c->heated)
+        return fail(c, NSC_EINVAL, "nsc_get_state_host_async: a temperature buffer was given, but the context has no temperature field (Ra = 0)");
     void* dst[5] = {ur, uth, uz, T, p};
-    int rc;
-    if (!c->copy_stream) {
-        for (int i = 0; i < 5; ++i)
-            if ((i != 3 || c->heated) && (rc = dev_alloc(c, &c->snap[i], c->F, false))) return rc;
-        NSC_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
-        NSC_CUDA(c, cudaEventCreateWithFlags(&c->ev_snap, cudaEventDisableTiming));
-        NSC_CUDA(c, cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming));
-        NSC_CUDA(c, cudaEventRecord(c->ev_copied, c->copy_stream));
-    }
+    int rc = transfer_setup(c, c->snap, &c->copy_stream, &c->ev_snap, &c->ev_copied, true, &c->down_ready);
+    if (rc) return rc;
     const size_t bytes = c->F * sizeof(cd);
     NSC_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied, 0));        // the previous snapshot has left
     for (int i = 0; i < 5; ++i)
@@ -336,15 +350,8 @@ int nsc_set_state_host_async(nsc_ctx* c, const void* ur, const void* uth, const 
     const void* src[5] = {ur, uth, uz, T, p};
     for (int i = 0; i < 3 + (c->heated ? 1 : 0); ++i)
         if (!src[i]) return fail(c, NSC_EINVAL, "nsc_set_state_host_async: required field pointer is NULL");
-    int rc;
-    if (!c->up_stream) {
-        for (int i = 0; i < 5; ++i)
-            if ((i != 3 || c->heated) && (rc = dev_alloc(c, &c->stage_in[i], c->F, false))) return rc;
-        NSC_CUDA(c, cudaStreamCreateWithFlags(&c->up_stream, cudaStreamNonBlocking));
-        NSC_CUDA(c, cudaEventCreateWithFlags(&c->ev_uploaded, cudaEventDisableTiming));
-        NSC_CUDA(c, cudaEventCreateWithFlags(&c->ev_staged_used, cudaEventDisableTiming));
-        NSC_CUDA(c, cudaEventRecord(c->ev_staged_used, c->stream));
-    }
+    int rc = transfer_setup(c, c->stage_in, &c->up_stream, &c->ev_uploaded, &c->ev_staged_used, false, &c->up_ready);
+    if (rc) return rc;
     const size_t bytes = c->F * sizeof(cd);
     NSC_CUDA(c, cudaStreamWaitEvent(c->up_stream, c->ev_staged_used, 0));     // the previous staging set has been taken over
     for (int i = 0; i < 5; ++i) {
@@ -365,8 +372,8 @@ int nsc_set_state_host_async(nsc_ctx* c, const void* ur, const void* uth, const 
 
 int nsc_host_copies_wait(nsc_ctx* c) {
     if (!c) return NSC_EINVAL;
-    if (c->up_stream) NSC_CUDA(c, cudaStreamSynchronize(c->up_stream));
-    if (c->copy_stream) NSC_CUDA(c, cudaStreamSynchronize(c->copy_stream));
+    if (c->up_ready) NSC_CUDA(c, cudaStreamSynchronize(c->up_stream));
+    if (c->down_ready) NSC_CUDA(c, cudaStreamSynchronize(c->copy_stream));
     return NSC_OK;
 }
 

@@ -94,7 +94,7 @@ struct nsc_ctx {
     double graph_dt = 0.0;
     cudaStream_t graph_stream = nullptr;
     long long graph_gen = -1, ptr_gen = 0, graph_launches = 0, graph_replays = 0;
-    int n_slices = 2;                                 // mode slices of the linear stage (NSC_LIN_SLICES overrides)
+    int n_slices = 2;                                 // mode slices of the linear stage (nsc_params.linear_slices)
     cudaStream_t slice_stream[NSC_MAX_SLICES] = {};   // their streams
     cudaEvent_t slice_ev[NSC_MAX_SLICES + 1] = {};    // [0] fork, [1 + s] join of slice s
     // NEXT-2 window (nsc_set_window): the nonlinear term is evaluated at the radial levels [wj0, wj1) only, the
@@ -105,10 +105,12 @@ struct nsc_ctx {
     nsc::cd* snap[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_snap = nullptr, ev_copied = nullptr;
+    bool down_ready = false;              // snapshot set, stream and both events exist (set last by the first-use set-up)
     // asynchronous host-to-device copies (nsc_set_state_host_async): staging set + private upload stream
     nsc::cd* stage_in[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     cudaStream_t up_stream = nullptr;
     cudaEvent_t ev_uploaded = nullptr, ev_staged_used = nullptr;
+    bool up_ready = false;                // likewise for the staging set
     bool have_state = false;
     std::string err;
     long long launches = 0;

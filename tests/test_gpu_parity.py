@@ -868,6 +868,19 @@ def test_double_buffered_host_transfers_equal_the_synchronous_ones(torch_cuda):
         for ref, out in zip(sync_out, pinned):
             for a, b in zip(ref, out):
                 np.testing.assert_array_equal(a, b)
+    # a temperature buffer handed to a context without temperature would stay unwritten: refused, not skipped
+    cold = synth.scaled_config(0, N_r=12, M=4, K=4)
+    with _ctx(cold) as ctx:
+        st = synth.make_state(cold, ctx.grid())
+        ctx.set_state(*st)
+        bufs = [np.full(st[0].shape, 7.0 + 0j) for _ in range(5)]
+        with pytest.raises(Exception, match="temperature"):
+            ctx.get_state_host_async(*bufs)
+        ctx.get_state_host_async(bufs[0], bufs[1], bufs[2], None, bufs[4])
+        ctx.host_copies_wait()
+        for i in (0, 1, 2, 4):
+            np.testing.assert_array_equal(bufs[i], st[i])
+        assert (bufs[3] == 7.0).all()
 
 
 def test_measured_fp64_peaks_are_sane_and_leave_the_current_device_alone(torch_cuda):
