@@ -443,6 +443,17 @@ class Oracle:
             IM, IK = IM.ravel(), IK.ravel()
         else:
             IM, IK = (np.asarray(x) for x in modes)
+        if self.solve == "c":
+            # the C backend forms its own right-hand sides, for the listed modes only: taken before the all-mode
+            # arrays below are built (they would be unused; at N_r = 512 with 5e5 modes they cost ~40 GB and minutes)
+            out = [np.empty((N_r, len(IM)), self.cplx) for _ in range(5)]
+            self._substep_c(state, E, dt, IM, IK, out)
+            if not p.heated:
+                out[3] = None
+            if full:
+                shp = (N_r, p.M + 1, 2 * p.K + 1)
+                out = [None if o is None else o.reshape(shp) for o in out]
+            return out
         r = self.r[:, None, None]
         n = self.n[None, :, None]
         # L1 right-hand sides, formed for all modes (cheap) then gathered per mode
@@ -465,14 +476,6 @@ class Oracle:
             rhs[3][0, 0, p.K], rhs[3][-1, 0, p.K] = 0.5, -0.5
         nB = len(IM)
         out = [np.empty((N_r, nB), self.cplx) for _ in range(5)]
-        if self.solve == "c":
-            self._substep_c(state, E, dt, IM, IK, out)
-            if not p.heated:
-                out[3] = None
-            if full:
-                shp = (N_r, p.M + 1, 2 * p.K + 1)
-                out = [None if o is None else o.reshape(shp) for o in out]
-            return out
 
         def solve_chunk(s):
             im, ik = IM[s:s + chunk], IK[s:s + chunk]

@@ -152,7 +152,7 @@ def test_nonlinear_broadband_random_fields_and_chunking(torch_cuda):
         with _ctx(cfg, radial_chunk=chunk) as ctx:
             ctx.set_state(*_dev(torch, fs), None)
             res.append(ctx.nonlinear_to_host())
-    assert rel_l2(res[0], ref) <= TOL_N
+    check_parity(res[0], ref, TOL_N, cfg["K"], "broadband random fields")
     for other in res[1:]:
         for a, b in zip(res[0], other):
             np.testing.assert_array_equal(a, b)
@@ -168,7 +168,7 @@ def test_nonlinear_padded_grid_variant(torch_cuda):
         st = synth.make_state(cfg, ctx.grid())
         ctx.set_state(*_dev(torch, st))
         got = ctx.nonlinear_to_host()
-    assert rel_l2(got, o.nonlinear(*st[:3])) <= TOL_N
+    check_parity(got, o.nonlinear(*st[:3]), TOL_N, cfg["K"], "cfg 1 on the 24 x 48 grid")
 
 
 SUB_CASES = [(0, 32, 8, 8), (2, 24, 4, 8), (1, 64, 8, 4), (3, 40, 4, 4), (2, 9, 4, 4)]
@@ -191,7 +191,7 @@ def test_substep_matches_oracle(torch_cuda, ci, N_r, M, K):
         ctx.substep(*Ed, cfg["dt"])
         got = ctx.state_to_host()
     ref = o.substep(st, E, cfg["dt"])
-    assert rel_l2(got[:nf], ref[:nf]) <= 1e-11
+    check_parity(got[:nf], ref[:nf], 1e-11, cfg["K"], f"sub-step {ci, N_r, M, K}")
     assert rel_l2([got[4]], [ref[4]]) <= 1e-7       # pressure: parity unpinned (phi / dt amplifies round-off)
 
 
@@ -379,7 +379,7 @@ def test_substep_uniform_grid_and_other_implicitness(torch_cuda, grid, c):
         ctx.substep(*_dev(torch, E), cfg["dt"])
         got = ctx.state_to_host()
         ref = o.substep(st, E, cfg["dt"])
-        assert rel_l2(got[:nf], ref[:nf]) <= 1e-11
+        check_parity(got[:nf], ref[:nf], 1e-11, cfg["K"], f"sub-step, grid {grid}, c = {c}")
         ctx.set_state(*_dev(torch, st))
         for _ in range(2):
             ctx.step(cfg["dt"])
@@ -387,7 +387,7 @@ def test_substep_uniform_grid_and_other_implicitness(torch_cuda, grid, c):
     ref = st
     for _ in range(2):
         ref = o.step(ref, cfg["dt"])
-    assert rel_l2(got[:nf], ref[:nf]) <= TOL_STEP
+    check_parity(got[:nf], ref[:nf], TOL_STEP, cfg["K"], f"two steps, grid {grid}, c = {c}")
 
 
 @pytest.mark.parametrize("ci,N_r,M,K,mult,amp,kmin", [(0, 24, 8, 8, 4.0, 5e-2, 2), (2, 20, 4, 8, 20.0, None, 1)])
@@ -423,11 +423,11 @@ def test_iterated_corrector_matches_oracle(torch_cuda, ci, N_r, M, K, mult, amp,
         ref, k_ref, err_ref = o.step_iterated(st, dt, tol, 30)
         assert k == k_ref and kmin <= k < 30
         assert abs(err - err_ref) <= 1e-3 * err_ref + 1e-15
-        assert rel_l2(got[:nf], ref[:nf]) <= TOL_STEP
+        check_parity(got[:nf], ref[:nf], TOL_STEP, cfg["K"], f"iterated corrector, {k} passes")
         ctx.step(dt)
         got2 = ctx.state_to_host()
     ref2 = o.step(ref, dt)
-    assert rel_l2(got2[:nf], ref2[:nf]) <= TOL_STEP
+    check_parity(got2[:nf], ref2[:nf], TOL_STEP, cfg["K"], "plain step after the iterated one")
 
 
 @pytest.mark.parametrize("ci,N_r,M,K", [(2, 24, 8, 8), (0, 20, 4, 8)])
@@ -480,9 +480,9 @@ def test_nonlinear_length_768_in_several_radial_chunks(torch_cuda, ci, N_r, M, K
 def test_full_size_cfg5_sampled(torch_cuda):
     """BASELINE.json configs[4] (the paper's Fig. 1 problem size: N_r = 512, 513 x 1025 modes, heated; 131 GB on
     the device, ~20 GB of host arrays) at full size: the nonlinear term at sampled radial nodes against the
-    oracle (70 s).  With NSC_TEST_CFG5_SUBSTEP=1 also one sub-step at sampled modes (the oracle forms the
-    right-hand sides of all 5e5 modes with dense 512 x 512 operators: 28 min; last run, round 1: nonlinear
-    rel-L2 1.0e-15, sub-step rel-L2 6.7e-13, recorded in DESIGN.md section 9)."""
+    naive-DFT oracle (70 s), then one sub-step with that term as the explicit term at sampled modes against the
+    oracle's plain-C backend (per listed mode: seconds; the dense backend forms the right-hand sides of all 5e5
+    modes with 512 x 512 operators, 28 min, which is why this leg used to be opt-in)."""
     import gc
     torch = torch_cuda
     free_dev = torch.cuda.mem_get_info()[0]
@@ -496,27 +496,25 @@ def test_full_size_cfg5_sampled(torch_cuda):
     o = oracle_of(cfg, dft="naive")
     N_r = cfg["N_r"]
     nodes = [0, N_r // 2 + 3, N_r - 1]
-    with_substep = bool(os.environ.get("NSC_TEST_CFG5_SUBSTEP"))
     rng = np.random.default_rng(12)
-    im = np.concatenate([[0, 0, cfg["M"], 1], rng.integers(0, cfg["M"] + 1, 12)])
-    ik = np.concatenate([[cfg["K"], cfg["K"] + 1, 0, cfg["K"] - 1], rng.integers(0, 2 * cfg["K"] + 1, 12)])
+    im = np.concatenate([[0, 0, cfg["M"], 1], rng.integers(0, cfg["M"] + 1, 28)])
+    ik = np.concatenate([[cfg["K"], cfg["K"] + 1, 0, cfg["K"] - 1], rng.integers(0, 2 * cfg["K"] + 1, 28)])
     with _ctx(cfg) as ctx:
         st = synth.make_state(cfg, ctx.grid())
         ctx.set_state(*st)
         E = ctx.nonlinear_to_host()
         ref = o.nonlinear(*st[:4], nodes=nodes)
         check_parity([g[nodes] for g in E], ref, TOL_N, cfg["K"], "cfg 5 nonlinear at sampled nodes")
-        if not with_substep:
-            return
         ctx.substep(*_dev(torch, E), cfg["dt"])
         sub = ctx.state_to_host()
     got_s = [f[:, im, ik].copy() for f in sub[:4]]
     del sub
     gc.collect()
-    ref_s = o.substep(st, E, cfg["dt"], modes=(im, ik))
-    err_s = rel_l2(got_s, ref_s[:4])
-    print("cfg 5 sampled: sub-step rel-L2", err_s)
-    assert err_s <= TOL_STEP
+    ref_s = oracle_of(cfg, dft="naive", solve="c").substep(st, E, cfg["dt"], modes=(im, ik))
+    mean = np.nonzero((im == 0) & (ik == cfg["K"]))[0]
+    # the bar of the sub-step at cfg 3 / 4 is 1e-11 (1e-10 without (0,0)); cond(P) grows like N_r^4 on the clustered grid,
+    # so at N_r = 512 the bar is ten times that -- still ten times below the 1e-9 this leg asserted while it was opt-in
+    check_parity(got_s, ref_s[:4], 1e-10, cfg["K"], f"cfg 5 sub-step at {len(im)} modes", mean_index=mean)
 
 
 def test_step_graph_replay_equals_plain_launches(torch_cuda):
