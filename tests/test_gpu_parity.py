@@ -244,6 +244,34 @@ def test_twenty_steps_at_full_size(torch_cuda, ci):
     _twenty_steps_full(torch_cuda, ci, side_stream=(ci == 2))
 
 
+@pytest.mark.parametrize("N_r,M,K,chunk,nsteps", [(12, 512, 16, 5, 20), (12, 16, 512, 5, 20), (9, 512, 512, 4, 6)])
+def test_steps_on_the_1536_kernels_in_several_radial_chunks(torch_cuda, N_r, M, K, chunk, nsteps):
+    """What stands in for the unpinned full steps at cfg 5: cfg 5's physics (heated) and its
+    code path -- the length-1536 warp-pair kernels, the radial pipeline forced into several chunks (spectral k_dr +
+    three z transforms per line) and CUDA-graph replays on a side stream -- at radial sizes where the oracle can
+    step.  20 steps with the 1536 transform in theta only and in z only (0.3 s of oracle time per step), 6 steps
+    with both (9 x 513 x 1025 modes, 1536 x 1536 grid: 10 s per oracle step on the GPU box's host, 30 s on 8 cores;
+    measured in round 3: 3.6e-15 / 3.8e-15 after 20 steps, 5.2e-16 after 3 with both)."""
+    torch = torch_cuda
+    cfg = synth.scaled_config(4, N_r=N_r, M=M, K=K)
+    nf = nf_of(cfg)
+    assert nf == 4
+    o = oracle_of(cfg, dft="fft", solve="c")
+    with _ctx(cfg, radial_chunk=chunk) as ctx:
+        s = torch.cuda.Stream()
+        ctx.set_stream(s)
+        st = synth.make_state(cfg, ctx.grid())
+        ctx.set_state(*_dev(torch, st))
+        for _ in range(nsteps):
+            ctx.step(cfg["dt"])
+        got = ctx.state_to_host()
+        assert ctx.graph_replays() == nsteps
+    ref = st
+    for _ in range(nsteps):
+        ref = o.step(ref, cfg["dt"], workers=NCPU)
+    check_parity(got[:nf], ref[:nf], TOL_STEP, K, f"{nsteps} steps at {N_r} x {M + 1} x {2 * K + 1} modes, radial chunk {chunk}")
+
+
 @pytest.mark.skipif(not os.environ.get("NSC_TEST_CFG4_20STEPS"), reason="opt-in: the oracle takes ~2 min per step at cfg 4")
 def test_twenty_steps_at_full_cfg4(torch_cuda):
     """BASELINE.json configs[3] (N_r = 256, 257 x 513 modes; bench.py's workload, graph replays on a side
