@@ -141,3 +141,26 @@ def test_extended_precision_oracle_and_the_round_off_floor():
     e, ep = rel_l2(a[:3], b[:3]), rel_l2_pert(a[:3], b[:3], cfg["K"])
     print(f"cfg 1 floor: double vs long double after 20 steps: R14 {e:.2e}, without (0,0) {ep:.2e}")
     assert e <= 1e-11 and ep <= 1e-9
+
+
+@pytest.mark.parametrize("ci,N_r", [(3, 256), (4, 512)])
+def test_round_off_floor_of_twenty_steps_at_full_radial_resolution(ci, N_r):
+    """The same floor where it matters (cond(P) ~ 1e13 at N_r = 256 on the clustered grid): cfg 4's
+    and cfg 5's physics and synthetic state at their full radial resolution, the low wavenumbers only (M = K = 4:
+    the per-mode systems are worst conditioned there; 45 modes), 20 steps in double and in long double.  What the
+    two precisions disagree by is the part of a GPU-against-oracle difference that no kernel can remove; it is
+    printed, and recorded in DESIGN.md section 9 beside the measured parity figures (cfg 4, 20 steps: 3.1e-12,
+    1.4e-10 without (0,0))."""
+    cfg = synth.scaled_config(ci, N_r=N_r, M=4, K=4)
+    nf = nf_of(cfg)
+    o64 = oracle_of(cfg, dft="fft", solve="banded")
+    o80 = oracle_of(cfg, dft="fft", solve="banded", real=np.longdouble)
+    st = synth.make_state(cfg, o64.r)
+    a, b = st, [None if f is None else f.astype(np.clongdouble) for f in st]
+    for _ in range(20):
+        a = o64.step(a, cfg["dt"])
+        b = o80.step(b, cfg["dt"])
+    e, ep = rel_l2(a[:nf], b[:nf]), rel_l2_pert(a[:nf], b[:nf], cfg["K"])
+    print(f"floor at N_r = {N_r}: double vs long double after 20 steps: R14 {e:.2e}, without (0,0) {ep:.2e}")
+    assert np.isfinite(e) and np.isfinite(ep)
+    assert e <= 1e-9 and ep <= 1e-8          # the floor itself stays below the 20-step criterion (R14) and its 10x companion
